@@ -1,0 +1,186 @@
+"""Pins for oracle step O6 (kernel tables) and the paper's Eq. 1-6: P5, P7, P8."""
+import os
+
+import numpy as np
+from scipy import integrate
+
+from oracle import kernels as ok, imaging as oi
+from helpers import base_params, MODE_WPROJ, MODE_AWPROJ_ADJOINT, MODE_AWPROJ_PAPER, MODE_MOSAIC_PB
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def test_pswf_is_eigenfunction_of_sinc_kernel():
+    """The order-0 prolate spheroidal function is the eigenfunction of the finite Fourier transform:
+    int_{-1}^{1} psi(t) exp(i c x t) dt = mu * psi(x) on [-1,1]  (textbook definition; pins pswf() against
+    something other than scipy's own evaluation of it)."""
+    c = np.pi * 7 / 2.0
+    xs = np.array([0.0, 0.2, 0.5, 0.8, 0.95])
+    vals = np.array([integrate.quad(lambda t: ok.pswf(t, 7) * np.cos(c * x * t), -1, 1, epsabs=1e-12)[0] for x in xs])
+    ratio = vals / ok.pswf(xs, 7)
+    assert np.allclose(ratio, ratio[0], rtol=2e-7)
+    assert ok.pswf(0.0, 7) == 1.0 and abs(ok.pswf(1.0, 7) - 1.92e-4) < 2e-6      # SURVEY 8(c) probe value
+
+
+def test_P5_pswf_table_is_self_fourier():
+    """P5: the PSWF kernel table equals mu' * psi(2 d / S) at tap offset d cells (self-Fourier property), so the
+    generator's sampling, sub-cell direction (d - o/O) and crop are right."""
+    params = base_params(support_min=7, support_max=7, oversample=8)
+    tabs, supports = ok.make_tables(params)
+    t = tabs[0][0, 0]                                   # [oy][ox][dy][dx]
+    assert list(supports) == [7] and t.shape == (8, 8, 7, 7)
+    assert np.max(np.abs(t.imag)) < 1e-12
+    d = np.arange(-3, 4)
+    peak = abs(t).max()
+    for oy in range(-4, 4):
+        for ox in range(-4, 4):
+            py = ok.pswf(2.0 * (d - oy / 8.0) / 7.0, 7)
+            px = ok.pswf(2.0 * (d - ox / 8.0) / 7.0, 7)
+            model = np.outer(np.where(np.abs(d - oy / 8.0) <= 3.5, py, 0), np.where(np.abs(d - ox / 8.0) <= 3.5, px, 0))
+            got = t[oy + 4, ox + 4].real
+            scale = got[3, 3] / model[3, 3]
+            assert np.max(np.abs(got - scale * model)) < 3e-3 * peak
+    # normalisation: zero-offset taps sum to 1; other offsets within the truncation error
+    assert abs(t[4, 4].sum() - 1.0) < 1e-12
+    assert np.max(np.abs(t.sum(axis=(2, 3)) - 1.0)) < 3e-4      # SURVEY probe: 1.000007 .. 0.99991 (worst at o = -O/2)
+
+
+def test_P7_w_kernel_identities():
+    params = base_params(grid_size=256, cell_size_rad=0.2 / 256, n_wplanes=4, w_max=150.0, support_min=9,
+                         support_max=15, oversample=4, kernel_mode=MODE_WPROJ)
+    tabs, supports = ok.make_tables(params)
+    assert list(supports) == [15, 13, 11, 9, 11, 13, 15]
+    pswf_tabs, _ = ok.make_tables(base_params(grid_size=256, cell_size_rad=0.2 / 256, support_min=9, support_max=9,
+                                              oversample=4))
+    assert np.array_equal(tabs[3], pswf_tabs[0])                   # plane 0 == plain PSWF kernel, bit for bit
+    # T_{-p}(delta) = conj(T_{+p}(-delta)): mirrored taps and mirrored sub-cell offsets (ox=-2 has no partner)
+    for p in (1, 2, 3):
+        tp, tm = tabs[3 + p][0, 0], tabs[3 - p][0, 0]
+        for oy in (-1, 0, 1):
+            for ox in (-1, 0, 1):
+                assert np.allclose(tm[oy + 2, ox + 2], np.conj(tp[-oy + 2, -ox + 2][::-1, ::-1]), atol=1e-13)
+    # Parseval: uncropped sum |Tfine|^2 is independent of w because |exp(i phi)| = 1
+    funcs = {k: f for k, _, f in ok.image_functions(params)}
+    e = [np.sum(np.abs(ok._fine_kernel(funcs[k][0, 0], 4)) ** 2) for k in (3, 4, 6)]
+    assert np.allclose(e, e[0], rtol=1e-12)
+    # w-term sign (Eq. 2): the kernel's image-domain phase at (l,m) is exp(-2 pi i w (n-1))
+    k, s, f = next(x for x in ok.image_functions(params) if x[0] == 6)
+    nk = f.shape[-1]
+    j = nk // 2 + 5
+    l = 5 * 0.2 / nk
+    expected = np.exp(-2j * np.pi * 150.0 * (np.sqrt(1 - 2 * l * l) - 1))
+    assert np.allclose(f[0, 0, j, j] / abs(f[0, 0, j, j]), expected, atol=1e-12)
+
+
+def test_P8_mueller_and_stokes():
+    ident = np.eye(2)
+    assert np.array_equal(ok.mueller(ident, ident), np.eye(4))                     # J = I  =>  M = I4
+    ji, jj = np.diag([1.2 + 0.1j, 0.9]), np.diag([1.1, 0.8 - 0.2j])
+    m = ok.mueller(ji, jj)
+    assert np.count_nonzero(m - np.diag(np.diag(m))) == 0                          # zero leakage => diagonal
+    assert np.allclose(np.diag(m), [ji[0, 0] * np.conj(jj[0, 0]), ji[0, 0] * np.conj(jj[1, 1]),
+                                    ji[1, 1] * np.conj(jj[0, 0]), ji[1, 1] * np.conj(jj[1, 1])])
+    # leakage lands off the diagonal at first order
+    jl = ok.jones_matrix([0.01, 0.02j], 0.0)
+    ml = ok.mueller(jl, jl)
+    assert abs(ml[0, 1] - np.conj(0.01)) < 1e-15 and abs(ml[0, 2] - 0.01) < 1e-15
+    # Eq. 4: unpolarised source XX = YY = 1, XY = YX = 0  ->  I = 1, Q = U = V = 0; pure XX -> I = Q = 1/2
+    assert np.allclose(ok.STOKES @ [1, 0, 0, 1], [1, 0, 0, 0])
+    assert np.allclose(ok.STOKES @ [1, 0, 0, 0], [0.5, 0.5, 0, 0])
+    assert np.allclose(ok.STOKES @ [0, 1, 1, 0], [0, 0, 1, 0])                     # U (reading G3)
+    assert np.allclose(ok.STOKES @ [0, -1j, 1j, 0], [0, 0, 0, -1])                 # V = i(YX - XY)/2
+    assert np.allclose(ok.STOKES @ np.linalg.inv(ok.STOKES), np.eye(4))
+    # Eq. 5: identity Mueller stays identity in the Stokes basis
+    assert np.allclose(ok.mueller_stokes(np.eye(4)), np.eye(4))
+
+
+def test_P8_eq6_closed_forms_and_fig1():
+    """Eq. 6: |B'| = |B| + beta/|B| >= 2 sqrt(beta) = eps max|B|, 1/B' = B*/(|B|^2+beta);
+    Fig. 1 numbers (tests/golden/fig1_eq6_divergence.txt)."""
+    x = np.linspace(-3, 3, 6001)
+    beam = np.sinc(x) ** 2                                         # np.sinc = sin(pi x)/(pi x)
+    eps = 0.02
+    mod = ok.eq6_modify(beam, eps)
+    beta = (eps / 2) ** 2
+    assert np.all(np.abs(mod) >= eps * 1.0 - 1e-12)
+    assert abs(np.abs(mod).min() - eps) < 1e-4                     # equality where |B| = (eps/2) max|B|
+    nz = beam > 1e-9
+    assert np.allclose(1 / mod[nz], beam[nz] / (beam[nz] ** 2 + beta), rtol=1e-12)
+    assert np.all(np.isfinite(1 / mod))                            # finite at the nulls x = +-1, +-2, +-3
+    golden = {}
+    for line in open(os.path.join(GOLDEN, "fig1_eq6_divergence.txt")):
+        if not line.startswith("#") and line.strip():
+            name, val, used = line.split()
+            golden[name] = (float(val), used == "yes")
+    div = 1 - (1 / mod) / (1 / np.where(nz, beam, 1))              # fractional divergence of the inverse
+    centre = div[3000]
+    assert golden["centre"][1] and abs(centre / golden["centre"][0] - 1) < 0.01
+    side = (x > 1.2) & (x < 1.7)
+    k = np.argmax(np.where(side, beam, 0))                         # first sidelobe peak of sinc^2
+    assert golden["first_sidelobe"][1] and abs(div[k] / golden["first_sidelobe"][0] - 1) < 0.15
+    half = np.argmin(np.abs(beam - 0.5) + (x < 0))
+    assert abs(div[half] - 4e-4) < 2e-5 and not golden["half_power"][1]     # printed 4e-3 is a typo (G7)
+
+
+def test_eq1_single_pointing_and_airy():
+    b = ok.airy(np.linspace(0, 0.02, 50), 12.0, 1.0e9) ** 2
+    g = oi.mosaic_gamma(b[None])
+    assert np.allclose(g, (b / b.max()) / b ** 2)
+    assert ok.airy(0.0, 12.0, 1e9) == 1.0
+    first_null = 1.2196699 * 0.299792458 / 12.0                    # 1.22 lambda / D
+    assert abs(ok.airy(first_null, 12.0, 1e9)) < 1e-6
+
+
+def test_awproj_tables_structure():
+    """ADJOINT tables are (M S^-1)^H element by element times the scalar w-kernel; PAPER-mode gridding tables
+    invert the regularised Stokes Mueller matrix: with zero leakage and a flat beam they reduce to S itself."""
+    common = dict(grid_size=128, cell_size_rad=0.02 / 128, n_corr=4, n_pol=4, n_wplanes=2, w_max=50.0,
+                  support_min=7, support_max=9, oversample=2, n_aplanes=2, pa_rad=[0.1, 0.7],
+                  pointing_lm=[[0, 0]] * 2, leakage=[0.01 * np.exp(0.3j), 0.01 * np.exp(2.1j)])
+    pa = base_params(kernel_mode=MODE_AWPROJ_ADJOINT, dish_diameter_m=0.0, **common)      # D = 0: E = 1
+    tabs, supports = ok.make_tables(pa)
+    assert len(tabs) == 6 and list(supports) == [9, 7, 9, 9, 7, 9]
+    wp = base_params(kernel_mode=MODE_WPROJ, **{**common, "n_corr": 1, "n_pol": 1, "n_aplanes": 1,
+                                                   "pa_rad": [0.0], "pointing_lm": [[0, 0]]})
+    wt, _ = ok.make_tables(wp)
+    for a in range(2):
+        jm = ok.jones_matrix(pa["leakage"], pa["pa_rad"][a])
+        f = np.conj((ok.mueller(jm, jm) @ np.linalg.inv(ok.STOKES)).T)
+        for k in range(3):
+            scale = tabs[1][0, 0, 1, 1].sum() / wt[1][0, 0, 1, 1].sum() / f0(pa)          # global normalisation
+            for s in range(4):
+                for c in range(4):
+                    assert np.allclose(tabs[a * 3 + k][s, c], f[s, c] * wt[k][0, 0] * scale, atol=1e-13)
+    pp = base_params(kernel_mode=MODE_AWPROJ_PAPER, dish_diameter_m=0.0, beam_eps=0.2,
+                     **{**common, "leakage": [0j, 0j], "pa_rad": [0.0, 0.0]})
+    tg, _ = ok.make_tables(pp, "grid")
+    # flat beam B = 1: Eq. 6 gives B' = 1 + (eps/2)^2, so (M^S')^-1 S = S / 1.01 up to the global scale
+    ratio = tg[1] / tg[1][0, 0][None, None]
+    for s in range(4):
+        for c in range(4):
+            assert np.allclose(ratio[s, c][abs(tg[1][0, 0]) > 1e-9], ok.STOKES[s, c] / ok.STOKES[0, 0], atol=1e-9)
+    td, _ = ok.make_tables(pp, "degrid")
+    ta, _ = ok.make_tables(dict(pp, kernel_mode=MODE_AWPROJ_ADJOINT))
+    assert all(np.array_equal(x, y) for x, y in zip(td, ta))
+
+
+def f0(params):
+    jm = ok.jones_matrix(params["leakage"], params["pa_rad"][0])
+    return np.conj((ok.mueller(jm, jm) @ np.linalg.inv(ok.STOKES)).T)[0, 0]
+
+
+def test_P12_mosaic_flat_beam_equals_pswf():
+    pm = base_params(kernel_mode=MODE_MOSAIC_PB, dish_diameter_m=0.0)
+    pp = base_params()
+    tm, _ = ok.make_tables(pm)
+    tp, _ = ok.make_tables(pp)
+    assert np.array_equal(tm[0], tp[0])
+    # an off-centre pointing multiplies the image-domain function by the shifted power beam
+    pm2 = base_params(kernel_mode=MODE_MOSAIC_PB, n_aplanes=2, pa_rad=[0, 0], pointing_lm=[[0, 0], [0.004, -0.002]],
+                      freq_hz=3e9)
+    fs = list(ok.image_functions(pm2))
+    nk = fs[0][2].shape[-1]
+    l1 = (np.arange(nk) - nk // 2) * 0.064 / nk
+    ll, mm = np.meshgrid(l1, l1)
+    ratio = fs[1][2][0, 0][1:, 1:] / fs[0][2][0, 0][1:, 1:] * ok.airy(np.hypot(ll, mm), 12, 3e9)[1:, 1:] ** 2
+    assert np.allclose(ratio, ok.airy(np.hypot(ll - 0.004, mm + 0.002), 12, 3e9)[1:, 1:] ** 2, rtol=1e-9, atol=1e-12)
