@@ -1,0 +1,148 @@
+/* imager.h -- C-ABI of libimager.so: the gridding / degridding hot path of the GPU imager of
+ * arxiv/paper_2206_15117 ("A GPU-based Imager with Polarised Primary-beam Correction"), built for one
+ * NVIDIA B200 (sm_100a).  Citations "P:NN" are lines of the paper text; "R<n>" are the readings
+ * listed in DESIGN.md where the paper is silent.
+ *
+ * What is computed:
+ *   gridding    G[s][gy+dy][gx+dx] += sum_c T[kset][s][c][oy][ox][dy][dx] * (w_kc * V_kc)
+ *   degridding  V_kc = sum_s sum_{dy,dx} conj(T_d[kset][s][c][oy][ox][dy][dx]) * G[s][gy+dy][gx+dx]
+ * with T = anti-aliasing function x w-correction term x Mueller-matrix cell (or its inverse), Fourier
+ * transformed to the UV domain, oversampled O times per cell and looked up at the nearest sub-cell.
+ * (gx,gy), (ox,oy), the signed w-plane and the kernel set `kset` of a visibility follow R2-R5.
+ *
+ * General rules
+ *   - Every pointer argument says "dev" (CUDA device memory, caller-owned, e.g. a torch tensor) or "host".
+ *   - The library never allocates or frees caller memory.  All device work is enqueued on the given
+ *     cuda_stream (a cudaStream_t passed as void*; NULL = the legacy default stream).  The hot calls
+ *     (imager_grid / imager_degrid) never synchronise the device; plan creation and the debug exports do.
+ *   - Every call returns 0 on success or a negative imager_status.  No exceptions, no abort, no printing.
+ *     imager_last_error() gives a thread-local message for the last failure on this thread.
+ *     Asynchronous CUDA faults surface on the next call or at the caller's synchronisation.
+ *   - There is no CPU fallback: without a CUDA device every call fails with IMAGER_ERR_CUDA.
+ */
+#ifndef IMAGER_H_
+#define IMAGER_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum imager_status {
+    IMAGER_OK = 0,
+    IMAGER_ERR_INVALID_ARG = -1,
+    IMAGER_ERR_UNSUPPORTED = -2,
+    IMAGER_ERR_NOMEM = -3,
+    IMAGER_ERR_CUDA = -4,
+    IMAGER_ERR_TOO_MANY_VIS = -5
+} imager_status;
+
+/* kernel_mode: which image-domain function the kernel tables are the transform of (R6, R9-R11) */
+enum {
+    IMAGER_MODE_DELTA = 0,          /* S = 1, O = 1, T = 1 (test mode: a visibility lands on one cell)            */
+    IMAGER_MODE_PSWF = 1,           /* psi(l) psi(m): prolate-spheroidal anti-aliasing function only        */
+    IMAGER_MODE_WPROJ = 2,          /* psi psi exp(-2 pi i w_p (n-1)): w-projection                          */
+    IMAGER_MODE_AWPROJ_ADJOINT = 3, /* 4x4: (M S^-1)^H cells x psi psi x w-term; degridding is the exact adjoint   */
+    IMAGER_MODE_AWPROJ_PAPER = 4,   /* 4x4: gridding from (M^S')^-1 S with Eq. 6, degridding as mode 3  */
+    IMAGER_MODE_MOSAIC_PB = 5,      /* psi psi E^2(l - l_a, m - m_a): primary beam as gridding kernel       */
+    IMAGER_MODE_USER = 6            /* tables supplied by the caller                                               */
+};
+
+/* flags of imager_grid / imager_degrid */
+enum {
+    IMAGER_REUSE_INDEX = 1u,        /* uvw / a_index / nvis unchanged since the previous grid or degrid call on this
+                                       plan: skip indexing and bucketing (the steady state of a major-cycle loop) */
+    IMAGER_PATH_REFERENCE = 2u      /* use the simple one-warp-per-visibility kernels instead of the tiled ones
+                                       (same results up to summation order; for tests and A/B timing)             */
+};
+
+typedef struct imager_plan imager_plan;   /* opaque, owned by the library */
+
+/* Plain data, copied at imager_plan_create; the caller may free it (and what it points to) afterwards. */
+typedef struct imager_params {
+    int32_t grid_size;        /* N (even): grids are [n_pol][N][N] complex64, row-major, u = v = 0 at cell (N/2, N/2)  */
+    int32_t n_corr;           /* 1 or 4 correlations per visibility, order XX*, XY*, YX*, YY*                   */
+    int32_t n_pol;            /* 1 or 4 output grids, order I, Q, U, V (Eq. 4-5)                             */
+    int32_t n_wplanes;        /* P >= 1 planes in |w| from 0 to w_max ("configurable number of w-planes"; R4)    */
+    int32_t support_min;      /* taps per side on plane 0                                                              */
+    int32_t support_max;      /* taps per side on plane P-1; S_p per R5; (support_max - support_min) must be even     */
+    int32_t oversample;       /* O sub-cells per cell (even, or 1)                                                     */
+    int32_t n_aplanes;        /* A-planes: parallactic-angle bins or mosaic pointings (P:90 averaging; R12); >= 1     */
+    int32_t kernel_mode;      /* IMAGER_MODE_*                                                                         */
+    int32_t pswf_support;     /* S_ps of the anti-aliasing function psi = S00(pi S_ps / 2, eta); 0 means 7            */
+    double cell_size_rad;     /* image cell in radians; the uv cell is 1 / (N * cell) wavelengths                      */
+    double w_max;             /* wavelengths; ignored if P == 1                                                        */
+    double dish_diameter_m;   /* Airy beam E = 2 J1(x)/x, x = pi D rho / lambda (AWPROJ_*, MOSAIC_PB)                  */
+    double freq_hz;           /* frequency the beam is evaluated at                                                    */
+    double leakage[4];        /* d1.re, d1.im, d2.re, d2.im of D = [[1, d1], [d2, 1]] (AWPROJ_*)                       */
+    double beam_eps;          /* epsilon of Eq. 6, AWPROJ_PAPER only; 0 means 0.2                              */
+    const double* pa_rad;     /* host [n_aplanes] parallactic angle per A-plane (AWPROJ_*), or NULL = zeros           */
+    const double* pointing_lm;/* host [n_aplanes][2] pointing offsets (l, m) in radians (MOSAIC_PB), or NULL = zeros  */
+    const float* user_tables;        /* host, USER mode: gridding tables, complex64 interleaved, the sets
+                                        kset = a*(2P-1) + (sp+P-1) back to back, each [n_pol][n_corr][O][O][S][S]     */
+    const float* user_tables_degrid; /* host, USER mode: degridding tables in the same layout, or NULL = same tables  */
+    int64_t max_nvis;         /* scratch is sized for this many visibilities per call                                  */
+} imager_params;
+
+/* 16-byte index record of one visibility (R2-R5, R8); exported by imager_debug_index, compared bit-exactly
+ * with the oracle. */
+typedef struct imager_record {
+    int32_t gx, gy;           /* grid cell of the visibility (may lie outside the grid if dropped)                     */
+    uint32_t sub;             /* (ox + O/2) | (oy + O/2) << 8 | drop << 16                                             */
+    int32_t kset;             /* kernel set a*(2P-1) + (sp + P-1)                                                      */
+} imager_record;
+
+/* Create a plan: validates params, builds the kernel tables on the device (or uploads USER tables) and
+ * allocates scratch for max_nvis visibilities.  Synchronises cuda_stream before returning.
+ * Errors: INVALID_ARG (bad sizes, NULL), UNSUPPORTED (mode / shape combination not built), NOMEM, CUDA. */
+int imager_plan_create(const imager_params* params, void* cuda_stream, imager_plan** out_plan);
+
+/* Gridding.  Accumulates into `grid` (the caller zeroes it); visibilities whose footprint leaves the
+ * grid are skipped and counted (R8).  uvw dev float32 [nvis][3] in wavelengths ("baseline vectors ... in
+ * units of wavelength"); vis dev complex64 [nvis][n_corr]; weights dev float32 [nvis][n_corr]; a_index dev
+ * int32 [nvis] in [0, n_aplanes) or NULL (= 0); grid dev complex64 [n_pol][N][N]; sum_weights dev double
+ * [n_corr] or NULL, accumulated with the weights of the kept visibilities.
+ * Errors: INVALID_ARG, TOO_MANY_VIS (nvis > max_nvis), CUDA. */
+int imager_grid(imager_plan* plan, int64_t nvis, const float* uvw, const float* vis, const float* weights,
+                const int32_t* a_index, float* grid, double* sum_weights, uint32_t flags, void* cuda_stream);
+
+/* Degridding: predicts vis_out dev complex64 [nvis][n_corr] (overwritten, input order) from grid dev
+ * complex64 [n_pol][N][N]; dropped visibilities predict 0.  Weights play no part. */
+int imager_degrid(imager_plan* plan, int64_t nvis, const float* uvw, const int32_t* a_index, const float* grid,
+                  float* vis_out, uint32_t flags, void* cuda_stream);
+
+/* Destroy a plan and free everything it owns.  NULL is a no-op. */
+int imager_plan_destroy(imager_plan* plan);
+
+/* ---- surrounding stages, built but outside the timed hot path (BASELINE.json north_star item 3) ---- */
+
+/* direction = +1: grid -> image: centred forward DFT (cuFFT) of each [N][N] plane in place, then divide by
+ * psi(l) psi(m) and by norm (pass the sum of weights; 0 means 1).  direction = -1: image -> grid: divide by
+ * psi psi, then the centred unnormalised inverse DFT (R1: signs follow Eq. 2).  data dev complex64. */
+int imager_grid_image_transform(imager_plan* plan, float* data, int32_t direction, double norm, void* cuda_stream);
+
+/* ---- test / debug exports (synchronise; not part of the hot path) ---- */
+
+/* Runs indexing + bucketing for (uvw, a_index) and copies out: records host [nvis], perm host int32 [nvis]
+ * (sorted position -> input index, stable), sorted keys host uint32 [nvis], bucket_offset host int32
+ * [n_buckets + 1] (see imager_plan_info), n_kept.  Any output pointer may be NULL. */
+int imager_debug_index(imager_plan* plan, int64_t nvis, const float* uvw, const int32_t* a_index,
+                       imager_record* records_out, int32_t* perm_out, uint32_t* keys_out,
+                       int32_t* bucket_offset_out, int64_t* n_kept_out, void* cuda_stream);
+
+/* Copies kernel set `kset` (gridding tables if which == 0, degridding if 1) to host_out in the canonical
+ * layout [n_pol][n_corr][O][O][S][S] complex64 and writes its support S.  host_out may be NULL (size query). */
+int imager_debug_kernels(imager_plan* plan, int32_t kset, int32_t which, float* host_out, int32_t* support_out);
+
+/* info: [0] n_sets, [1] bucket tile size, [2] n_buckets, [3] key bits, [4] dropped visibilities of the last
+ * indexing (synchronises), [5] GPU kernel launches issued by the last imager_grid / imager_degrid call. */
+int imager_plan_info(imager_plan* plan, int64_t info_out[8]);
+
+/* Thread-local message of the last failing call on this thread ("" if none); valid until the next call. */
+const char* imager_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* IMAGER_H_ */

@@ -6,7 +6,7 @@
  *   O4  for k in input order, not dropped:  val_c = w_kc * V_kc
  *         G[s][gy+dy][gx+dx] += sum_c T[kset_k][s][c][oy][ox][dy][dx] * val_c      (complex128 accumulation)
  *         A[s][gy+dy][gx+dx] += sum_c |T| * |val_c|                                  (parity normaliser)
- *         sumwt[c] += w_kc
+ *         sumwt[c] += w_kc                                                         (kept visibilities only)
  *   O5  V_kc = sum_s sum_{dy,dx} conj(T[kset_k][s][c][oy][ox][dy][dx]) * G[s][gy+dy][gx+dx],
  *         B_kc = sum |T| * |G|;  dropped visibilities predict 0.
  *
@@ -112,8 +112,9 @@ int oracle_grid(int64_t nvis, int N, int n_corr, int n_pol, int O,
             }
         }
     }
-    for (int64_t k = 0; k < nvis; ++k)
-        for (int c = 0; c < n_corr; ++c) sumwt[c] += (double)weights[k * n_corr + c];
+    for (int64_t k = 0; k < nvis; ++k)                              /* dropped visibilities carry no weight (R8) */
+        if (!drop[k])
+            for (int c = 0; c < n_corr; ++c) sumwt[c] += (double)weights[k * n_corr + c];
     return 0;
 }
 

@@ -89,14 +89,17 @@ def bucket_keys(rec: dict, params: dict, tile: int) -> np.ndarray:
     return np.where(rec["drop"], np.int64(KEY_DROP), key).astype(np.uint32)
 
 
-def bucket_sort(keys: np.ndarray, oversample: int) -> dict:
-    """Stable sort by key; buckets are runs of equal key // O^2 (= kernel set x tile), dropped excluded.
-    Returns perm (int32, sorted position -> input index), sorted keys, and the compact bucket list
-    (bucket id, start) with a final sentinel start = number of kept visibilities."""
+def bucket_sort(keys: np.ndarray, params: dict, tile: int) -> dict:
+    """Stable sort by key; bucket b = key // O^2 (= (kset * nty + ty) * ntx + tx), dropped excluded.
+    Returns perm (int32, sorted position -> input index), the sorted keys, n_kept, and the dense
+    bucket_offset[n_buckets + 1] (bucket b occupies sorted positions bucket_offset[b] .. bucket_offset[b+1])."""
+    o = int(params["oversample"])
+    nt = -(-int(params["grid_size"]) // tile)
+    n_sets = int(params["n_aplanes"]) * (2 * int(params["n_wplanes"]) - 1)
+    n_buckets = n_sets * nt * nt
     perm = np.argsort(keys, kind="stable").astype(np.int32)
     skeys = keys[perm]
     n_kept = int(np.searchsorted(skeys, KEY_DROP, side="left"))
-    bid = (skeys[:n_kept].astype(np.int64)) // (oversample * oversample)
-    starts = np.flatnonzero(np.concatenate([[True], bid[1:] != bid[:-1]])) if n_kept else np.zeros(0, np.int64)
-    return dict(perm=perm, sorted_keys=skeys, n_kept=n_kept, bucket_id=bid[starts].astype(np.int64),
-                bucket_start=np.concatenate([starts, [n_kept]]).astype(np.int64))
+    edges = np.arange(n_buckets + 1, dtype=np.int64) * (o * o)
+    offsets = np.searchsorted(skeys[:n_kept].astype(np.int64), edges, side="left").astype(np.int32)
+    return dict(perm=perm, sorted_keys=skeys, n_kept=n_kept, bucket_offset=offsets)

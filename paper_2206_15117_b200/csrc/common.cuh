@@ -1,0 +1,90 @@
+// common.cuh -- internal declarations shared by the translation units of libimager.so (sm_100a only).
+// Nothing here is part of the C-ABI (include/imager.h is).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+#include "../../include/imager.h"
+
+namespace imager {
+
+constexpr int kBucketTile = 32;          // bucketing tile (cells); DESIGN.md "Bucketing key"
+constexpr uint32_t kKeyDrop = 0xFFFFFFFFu;
+constexpr int kSortChunk = 2048;         // items per warp in the radix sort
+constexpr int kNumSMs = 148;             // B200
+
+void set_error(const char* fmt, ...);
+int cuda_fail(cudaError_t e, const char* what);
+
+#define IMAGER_CUDA(call)                                              \
+    do {                                                               \
+        cudaError_t e__ = (call);                                      \
+        if (e__ != cudaSuccess) return ::imager::cuda_fail(e__, #call); \
+    } while (0)
+
+}  // namespace imager
+
+struct imager_plan {
+    imager_params p;                     // copy of the caller's params (host pointers cleared)
+    int n_sets = 0, nt = 0, n_buckets = 0, key_bits = 0, sort_passes = 0;
+    double uv_scale = 0, w_scale = 0;
+    std::vector<int> plane_support;      // S_p, p = 0..P-1
+    std::vector<int64_t> set_offset;     // per kernel set, in complex elements (n_sets + 1)
+    std::vector<int> set_support;        // per kernel set
+
+    float2* d_tab_grid = nullptr;        // canonical layout, sets back to back
+    float2* d_tab_degrid = nullptr;      // == d_tab_grid unless the mode has separate degridding tables
+    int64_t* d_set_offset = nullptr;     // [n_sets + 1]
+    int32_t* d_set_support = nullptr;    // [n_sets]
+    int32_t* d_plane_support = nullptr;  // [P]
+
+    // index / bucketing state (valid for `indexed_nvis` visibilities once index_valid)
+    imager_record* d_rec = nullptr;      // [max_nvis] input order
+    uint32_t* d_key[2] = {nullptr, nullptr};
+    int32_t* d_perm[2] = {nullptr, nullptr};
+    int sorted_buf = 0;                  // which of d_key/d_perm holds the sorted result
+    int32_t* d_bucket_offset = nullptr;  // [n_buckets + 1]
+    int32_t* d_hist = nullptr;           // radix histograms [256 * n_warp_chunks]
+    int32_t* d_scan_tmp = nullptr;       // block sums of the scan, all levels
+    int64_t scan_tmp_len = 0;
+    int32_t* d_counters = nullptr;       // [0] n_kept, [1] n_dropped, [2..] work-queue heads
+    int64_t indexed_nvis = -1;
+    bool index_valid = false;
+
+    // tiled path work list
+    int32_t* d_items = nullptr;          // [max_items][4]
+    int64_t max_items = 0;
+
+    double* d_taper = nullptr;           // [N] psi(2(x-N/2)/N) for imager_grid_image_transform
+    void* fft_plan = nullptr;            // cufftHandle stored as intptr
+    bool fft_ready = false;
+
+    int last_launches = 0;
+};
+
+namespace imager {
+
+// index_sort.cu
+int run_index_and_sort(imager_plan* pl, int64_t nvis, const float* uvw, const int32_t* a_index, cudaStream_t st);
+
+// gridder_ref.cu
+int launch_grid_reference(imager_plan* pl, int64_t nvis, const float2* vis, const float* weights, float2* grid,
+                          cudaStream_t st);
+int launch_degrid_reference(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, cudaStream_t st);
+int launch_sum_weights(imager_plan* pl, int64_t nvis, const float* weights, double* sum_weights, cudaStream_t st);
+
+// gridder_tiled.cu
+bool tiled_supported(const imager_plan* pl);
+int launch_grid_tiled(imager_plan* pl, int64_t nvis, const float2* vis, const float* weights, float2* grid,
+                      cudaStream_t st);
+int launch_degrid_tiled(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, cudaStream_t st);
+
+// tables.cu
+int build_tables(imager_plan* pl, const imager_params* user, cudaStream_t st);
+
+// transform.cu
+int grid_image_transform(imager_plan* pl, float2* data, int direction, double norm, cudaStream_t st);
+void destroy_transform(imager_plan* pl);
+
+}  // namespace imager

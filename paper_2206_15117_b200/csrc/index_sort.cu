@@ -1,0 +1,213 @@
+// index_sort.cu -- hot-path steps A1 (index) and A2 (bucketing) of DESIGN.md.
+//
+// A1: one thread per visibility: uvw (float32, wavelengths) -> imager_record + 32-bit bucket key.
+//     Integer results are defined by DESIGN.md R2-R5/R8 and must equal the oracle bit for bit:
+//       q = rint(double(u) * uv_scale)            one IEEE multiply + round-half-even (cvt.rni.s64.f64)
+//       i = floor((q + O/2)/O), o = q - i*O, g = i + N/2;  p = min(P-1, rint(|w| * w_scale)), sp = sign(w) p
+//       kset = a*(2P-1) + sp + P-1;  drop if the S_p footprint leaves the grid
+//       key  = ((kset*nt + gy/32)*nt + gx/32)*O*O + (oy+O/2)*O + (ox+O/2), dropped -> 0xFFFFFFFF
+// A2: stable LSD radix sort (8-bit digits) of (key, input index), then dense bucket offsets by binary search.
+//     The sort is hand-written: per-warp chunk histograms -> exclusive scan -> stable per-warp scatter using
+//     __match_any_sync ranks.  Stability makes the permutation unique, hence comparable bit-exactly.
+#include "common.cuh"
+
+namespace imager {
+
+__device__ __forceinline__ long long floor_div(long long a, long long b) {
+    long long q = a / b;
+    return (a % b != 0 && ((a < 0) != (b < 0))) ? q - 1 : q;
+}
+
+__global__ void index_kernel(int64_t nvis, const float* __restrict__ uvw, const int32_t* __restrict__ a_index,
+                             double uv_scale, double w_scale, int N, int O, int P, int nt,
+                             const int32_t* __restrict__ plane_support, imager_record* __restrict__ rec,
+                             uint32_t* __restrict__ key, int32_t* __restrict__ perm, int32_t* __restrict__ counters) {
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nvis) return;
+    const float u = uvw[3 * k], v = uvw[3 * k + 1], w = uvw[3 * k + 2];
+    const long long qx = __double2ll_rn(__dmul_rn((double)u, uv_scale));
+    const long long qy = __double2ll_rn(__dmul_rn((double)v, uv_scale));
+    const int half_o = O / 2;
+    const long long ix = floor_div(qx + half_o, O), iy = floor_div(qy + half_o, O);
+    const int ox = (int)(qx - ix * O), oy = (int)(qy - iy * O);
+    const long long gx = ix + N / 2, gy = iy + N / 2;
+    long long p = __double2ll_rn(__dmul_rn(fabs((double)w), w_scale));
+    if (p > P - 1) p = P - 1;
+    const int sp = (w < 0.f) ? -(int)p : (int)p;
+    const int a = a_index ? a_index[k] : 0;
+    const int kset = a * (2 * P - 1) + sp + P - 1;
+    const int S = plane_support[p], h_lo = S / 2, h_hi = S - 1 - h_lo;
+    const bool drop = (gx - h_lo < 0) || (gx + h_hi >= N) || (gy - h_lo < 0) || (gy + h_hi >= N);
+    imager_record r;
+    r.gx = (int32_t)gx;
+    r.gy = (int32_t)gy;
+    r.sub = (uint32_t)(ox + half_o) | ((uint32_t)(oy + half_o) << 8) | ((uint32_t)drop << 16);
+    r.kset = kset;
+    rec[k] = r;
+    uint32_t kk = kKeyDrop;
+    if (!drop)
+        kk = (uint32_t)((((long long)kset * nt + gy / kBucketTile) * nt + gx / kBucketTile) * (O * O) +
+                        (oy + half_o) * O + (ox + half_o));
+    else
+        atomicAdd(&counters[1], 1);
+    key[k] = kk;
+    perm[k] = (int32_t)k;
+}
+
+// ---- radix sort: one warp owns kSortChunk consecutive items ----
+__global__ void radix_hist_kernel(int64_t n, const uint32_t* __restrict__ key, int shift, int32_t* __restrict__ hist,
+                                  int n_chunks) {
+    __shared__ int32_t cnt[4][256];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int chunk = blockIdx.x * 4 + warp;
+    for (int i = lane; i < 256; i += 32) cnt[warp][i] = 0;
+    __syncwarp();
+    if (chunk < n_chunks) {
+        const int64_t base = (int64_t)chunk * kSortChunk;
+        for (int i = lane; i < kSortChunk; i += 32) {
+            const int64_t idx = base + i;
+            if (idx < n) atomicAdd(&cnt[warp][(key[idx] >> shift) & 255u], 1);
+        }
+        __syncwarp();
+        for (int d = lane; d < 256; d += 32) hist[(int64_t)d * n_chunks + chunk] = cnt[warp][d];
+    }
+}
+
+__global__ void radix_scatter_kernel(int64_t n, const uint32_t* __restrict__ key_in, const int32_t* __restrict__ val_in,
+                                     uint32_t* __restrict__ key_out, int32_t* __restrict__ val_out, int shift,
+                                     const int32_t* __restrict__ hist_scanned, int n_chunks) {
+    __shared__ int32_t pos[4][256];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int chunk = blockIdx.x * 4 + warp;
+    if (chunk >= n_chunks) return;
+    for (int d = lane; d < 256; d += 32) pos[warp][d] = hist_scanned[(int64_t)d * n_chunks + chunk];
+    __syncwarp();
+    const int64_t base = (int64_t)chunk * kSortChunk;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    for (int i = 0; i < kSortChunk; i += 32) {
+        const int64_t idx = base + i + lane;
+        const bool live = idx < n;
+        const unsigned active = __ballot_sync(0xffffffffu, live);
+        if (live) {
+            const uint32_t kk = key_in[idx];
+            const int32_t vv = val_in[idx];
+            const unsigned d = (kk >> shift) & 255u;
+            const unsigned peers = __match_any_sync(active, d);
+            const int rank = __popc(peers & lt_mask);
+            const int dst = pos[warp][d] + rank;
+            __syncwarp(active);
+            if (rank == 0) pos[warp][d] += __popc(peers);
+            key_out[dst] = kk;
+            val_out[dst] = vv;
+        }
+        __syncwarp();
+    }
+}
+
+// ---- exclusive scan of int32 (1024 items per block), hierarchical ----
+__global__ void scan_block_kernel(const int32_t* in, int32_t* out, int32_t* __restrict__ sums,   // in may alias out
+                                  int64_t n) {
+    __shared__ int32_t warp_tot[8];
+    const int64_t base = (int64_t)blockIdx.x * 1024 + threadIdx.x * 4;
+    int32_t v[4], t = 0;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        v[j] = (base + j < n) ? in[base + j] : 0;
+        t += v[j];
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int32_t inc = t;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        int32_t y = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= d) inc += y;
+    }
+    if (lane == 31) warp_tot[warp] = inc;
+    __syncthreads();
+    int32_t woff = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) {
+        if (w < warp) woff += warp_tot[w];
+        total += warp_tot[w];
+    }
+    int32_t run = woff + inc - t;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        if (base + j < n) out[base + j] = run;
+        run += v[j];
+    }
+    if (threadIdx.x == 0 && sums) sums[blockIdx.x] = total;
+}
+
+__global__ void scan_add_kernel(int32_t* __restrict__ data, const int32_t* __restrict__ block_off, int64_t n) {
+    const int64_t i = (int64_t)blockIdx.x * 1024 + threadIdx.x;
+    const int32_t off = block_off[blockIdx.x];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const int64_t idx = i + j * 256;
+        if (idx < n) data[idx] += off;
+    }
+}
+
+static int exclusive_scan(imager_plan* pl, int32_t* data, int64_t n, int32_t* tmp, cudaStream_t st) {
+    const int64_t nb = (n + 1023) / 1024;
+    scan_block_kernel<<<(unsigned)nb, 256, 0, st>>>(data, data, nb > 1 ? tmp : nullptr, n);
+    pl->last_launches++;
+    if (nb > 1) {
+        int rc = exclusive_scan(pl, tmp, nb, tmp + nb, st);
+        if (rc) return rc;
+        scan_add_kernel<<<(unsigned)nb, 256, 0, st>>>(data, tmp, n);
+        pl->last_launches++;
+    }
+    return 0;
+}
+
+__global__ void bucket_offset_kernel(const uint32_t* __restrict__ skey, int64_t n, int n_buckets, int oo,
+                                     int32_t* __restrict__ bucket_offset, int32_t* __restrict__ counters) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b > n_buckets) return;
+    // lower_bound of b*O*O in the sorted keys (the drop key is larger than every bucket edge)
+    const uint64_t edge = (uint64_t)b * (uint64_t)oo;
+    int64_t lo = 0, hi = n;
+    while (lo < hi) {
+        const int64_t mid = (lo + hi) >> 1;
+        if ((uint64_t)skey[mid] < edge && skey[mid] != kKeyDrop) lo = mid + 1; else hi = mid;
+    }
+    bucket_offset[b] = (int32_t)lo;
+    if (b == n_buckets) counters[0] = (int32_t)lo;      // n_kept
+}
+
+int run_index_and_sort(imager_plan* pl, int64_t nvis, const float* uvw, const int32_t* a_index, cudaStream_t st) {
+    const imager_params& p = pl->p;
+    IMAGER_CUDA(cudaMemsetAsync(pl->d_counters, 0, 64 * sizeof(int32_t), st));
+    if (nvis > 0) {
+        index_kernel<<<(unsigned)((nvis + 255) / 256), 256, 0, st>>>(
+            nvis, uvw, a_index, pl->uv_scale, pl->w_scale, p.grid_size, p.oversample, p.n_wplanes, pl->nt,
+            pl->d_plane_support, pl->d_rec, pl->d_key[0], pl->d_perm[0], pl->d_counters);
+        pl->last_launches++;
+    }
+    int cur = 0;
+    const int n_chunks = (int)((nvis + kSortChunk - 1) / kSortChunk);
+    for (int pass = 0; pass < pl->sort_passes && nvis > 0; ++pass) {
+        const int shift = 8 * pass;
+        const unsigned blocks = (unsigned)((n_chunks + 3) / 4);
+        radix_hist_kernel<<<blocks, 128, 0, st>>>(nvis, pl->d_key[cur], shift, pl->d_hist, n_chunks);
+        pl->last_launches++;
+        int rc = exclusive_scan(pl, pl->d_hist, (int64_t)256 * n_chunks, pl->d_scan_tmp, st);
+        if (rc) return rc;
+        radix_scatter_kernel<<<blocks, 128, 0, st>>>(nvis, pl->d_key[cur], pl->d_perm[cur], pl->d_key[cur ^ 1],
+                                                     pl->d_perm[cur ^ 1], shift, pl->d_hist, n_chunks);
+        pl->last_launches++;
+        cur ^= 1;
+    }
+    pl->sorted_buf = cur;
+    bucket_offset_kernel<<<(unsigned)((pl->n_buckets + 1 + 255) / 256), 256, 0, st>>>(
+        pl->d_key[cur], nvis, pl->n_buckets, p.oversample * p.oversample, pl->d_bucket_offset, pl->d_counters);
+    pl->last_launches++;
+    IMAGER_CUDA(cudaGetLastError());
+    pl->indexed_nvis = nvis;
+    pl->index_valid = true;
+    return 0;
+}
+
+}  // namespace imager

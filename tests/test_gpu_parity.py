@@ -1,0 +1,191 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C-ABI binding, against the CPU oracle on the
+same seeded inputs.  Bar (BASELINE.json north_star): index / bucketing bit-exact; grids and degridded
+visibilities within 1e-5 of the oracle, normalised by sum |kernel . vis| per output element.
+
+The hot-path cases feed the ORACLE's kernel tables (rounded to complex64) to the library (USER mode), so that
+the comparison isolates indexing, bucketing, gridding and degridding; the library's own table generator is
+compared with the oracle's tables separately (test_gpu_tables.py)."""
+import numpy as np
+import pytest
+
+from oracle import index as oidx, gridder as og
+from helpers import (base_params, random_vis, oracle_tables, MODE_DELTA, MODE_PSWF, MODE_WPROJ, MODE_AWPROJ_ADJOINT,
+                     MODE_MOSAIC_PB)
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    return torch
+
+
+def _to_dev(torch, uvw, vis, wts, a):
+    d = lambda x: None if x is None else torch.from_numpy(np.ascontiguousarray(x)).cuda()
+    return d(uvw), d(vis), d(wts), d(a)
+
+
+def grid_error(g_gpu, oracle_out):
+    """max |G_gpu - G_oracle| / A[cell]; cells the oracle never touched must be exactly zero."""
+    g, a = oracle_out["grid"], oracle_out["norm"]
+    untouched = a == 0
+    assert np.all(g_gpu[untouched] == 0), "GPU wrote cells the oracle did not touch"
+    return float(np.max(np.abs(g_gpu[~untouched] - g[~untouched]) / a[~untouched])) if (~untouched).any() else 0.0
+
+
+def vis_error(v_gpu, oracle_out, drop):
+    v, b = oracle_out["vis"], oracle_out["norm"]
+    assert np.all(v_gpu[drop] == 0), "dropped visibilities must predict 0"
+    ok = b > 0
+    return float(np.max(np.abs(v_gpu[ok] - v[ok]) / b[ok])) if ok.any() else 0.0
+
+
+CASES = {
+    "pswf": lambda: base_params(grid_size=128, oversample=8),
+    "wproj": lambda: base_params(grid_size=256, oversample=4, n_wplanes=8, w_max=90.0, support_min=7, support_max=21,
+                                 kernel_mode=MODE_WPROJ, cell_size_rad=0.1 / 256),
+    "wproj_big_support": lambda: base_params(grid_size=256, oversample=2, n_wplanes=3, w_max=30.0, support_min=33,
+                                             support_max=67, kernel_mode=MODE_WPROJ, cell_size_rad=0.05 / 256),
+    "awproj": lambda: base_params(grid_size=128, oversample=4, n_wplanes=3, w_max=30.0, support_min=7, support_max=11,
+                                  n_corr=4, n_pol=4, n_aplanes=3, pa_rad=[0.0, 0.5, 1.0], pointing_lm=[[0, 0]] * 3,
+                                  leakage=[0.01j, -0.01], kernel_mode=MODE_AWPROJ_ADJOINT, cell_size_rad=0.04 / 128),
+    "mosaic_even": lambda: base_params(grid_size=128, oversample=4, support_min=16, support_max=16, n_aplanes=5,
+                                       pa_rad=[0] * 5, pointing_lm=[[0, 0], [0.003, 0.001], [-0.002, 0.004], [0.001, -0.003],
+                                                                    [0.0, 0.002]],
+                                       kernel_mode=MODE_MOSAIC_PB, cell_size_rad=0.03 / 128, freq_hz=3.0e9),
+}
+
+
+@pytest.mark.parametrize("case", sorted(CASES))
+@pytest.mark.parametrize("flags", [0, 2], ids=["default", "reference"])
+def test_grid_and_degrid_parity_small(torch_cuda, oracle_lib, case, flags):
+    torch = torch_cuda
+    from paper_2206_15117_b200 import Plan
+    params = CASES[case]()
+    nvis = 6000
+    uvw, vis, wts, a = random_vis(params, nvis, seed=31, frac=0.52, a_planes=params["n_aplanes"] > 1)
+    wts[::17] = 0.0                                                  # zero weights contribute nothing (R9)
+    _, _, flat, offs = oracle_tables(params)
+    rec = oidx.index_visibilities(uvw, a, params)
+    assert rec["drop"].any() and (~rec["drop"]).sum() > nvis // 4      # frac 0.52 pushes some footprints off the grid
+    n, npol, nc = params["grid_size"], params["n_pol"], params["n_corr"]
+    with Plan(params, nvis, user_tables=flat) as plan:
+        d_uvw, d_vis, d_wts, d_a = _to_dev(torch, uvw, vis, wts, a)
+        grid = torch.zeros((npol, n, n), dtype=torch.complex64, device="cuda")
+        sumwt = torch.zeros(nc, dtype=torch.float64, device="cuda")
+        plan.grid(d_uvw, d_vis, d_wts, grid, d_a, sumwt, flags=flags)
+        torch.cuda.synchronize()
+        ref = og.grid(rec, vis, wts, flat, offs, params)
+        err = grid_error(grid.cpu().numpy(), ref)
+        assert err <= TOL, f"grid parity {err:.3e}"
+        assert np.allclose(sumwt.cpu().numpy(), ref["sumwt"], rtol=1e-12)
+        assert plan.info()["n_dropped"] == int(rec["drop"].sum())
+        # warm call (index reuse) accumulates a second copy
+        plan.grid(d_uvw, d_vis, d_wts, grid, d_a, None, flags=flags | 1)
+        torch.cuda.synchronize()
+        ref2 = dict(grid=2 * ref["grid"], norm=2 * ref["norm"])
+        assert grid_error(grid.cpu().numpy(), ref2) <= TOL
+        # degridding from a random grid
+        rng = np.random.default_rng(9)
+        g = (rng.standard_normal((npol, n, n)) + 1j * rng.standard_normal((npol, n, n))).astype(np.complex64)
+        d_g = torch.from_numpy(g).cuda()
+        out = torch.full((nvis, nc), 7.0 + 7.0j, dtype=torch.complex64, device="cuda")
+        plan.degrid(d_uvw, d_g, out, d_a, flags=flags)
+        torch.cuda.synchronize()
+        refd = og.degrid(rec, g, flat, offs, params)
+        errd = vis_error(out.cpu().numpy(), refd, rec["drop"])
+        assert errd <= TOL, f"degrid parity {errd:.3e}"
+
+
+@pytest.mark.parametrize("case", sorted(CASES))
+def test_index_and_bucketing_bit_exact(torch_cuda, case):
+    torch = torch_cuda
+    from paper_2206_15117_b200 import Plan
+    params = CASES[case]()
+    nvis = 50000
+    uvw, _, _, a = random_vis(params, nvis, seed=41, frac=0.55, a_planes=params["n_aplanes"] > 1)
+    # exact ties on the fine lattice (q + 0.5) in both signs
+    uv_scale = float(params["oversample"]) * float(params["grid_size"]) * params["cell_size_rad"]
+    uvw[:64, 0] = ((np.arange(64) - 32) + 0.5) / uv_scale
+    uvw[:64, 1] = -uvw[:64, 0]
+    _, _, flat, _ = oracle_tables(params)
+    rec = oidx.index_visibilities(uvw, a, params)
+    keys = oidx.bucket_keys(rec, params, tile=32)
+    ref = oidx.bucket_sort(keys, params, tile=32)
+    with Plan(params, nvis, user_tables=flat) as plan:
+        assert plan.info()["bucket_tile"] == 32
+        d_uvw, _, _, d_a = _to_dev(torch, uvw, None, None, a)
+        got = plan.debug_index(d_uvw, d_a)
+    assert np.array_equal(got["records"], oidx.pack_records(rec, params["oversample"]))
+    assert np.array_equal(got["sorted_keys"], ref["sorted_keys"])
+    assert np.array_equal(got["perm"], ref["perm"])
+    assert got["n_kept"] == ref["n_kept"]
+    assert np.array_equal(got["bucket_offset"], ref["bucket_offset"])
+
+
+def test_delta_kernel_single_visibility(torch_cuda):
+    """P1 on the GPU: one visibility, delta kernel, lands on the expected cell with value w*V."""
+    torch = torch_cuda
+    from paper_2206_15117_b200 import Plan
+    n, cell = 64, 1.0e-3
+    du = 1.0 / (n * cell)
+    params = base_params(grid_size=n, cell_size_rad=cell, support_min=1, support_max=1, oversample=1, kernel_mode=MODE_DELTA)
+    with Plan(params, 4) as plan:
+        uvw = torch.tensor([[3.2 * du, -7.6 * du, 0.0]], dtype=torch.float32, device="cuda")
+        vis = torch.tensor([[2.0 - 3.0j]], dtype=torch.complex64, device="cuda")
+        wts = torch.tensor([[0.25]], dtype=torch.float32, device="cuda")
+        grid = torch.zeros((1, n, n), dtype=torch.complex64, device="cuda")
+        plan.grid(uvw, vis, wts, grid)
+        g = grid.cpu().numpy()[0]
+        assert np.count_nonzero(g) == 1 and g[n // 2 - 8, n // 2 + 3] == np.complex64(0.25 * (2 - 3j))
+
+
+def test_edge_cases_empty_and_all_dropped(torch_cuda):
+    torch = torch_cuda
+    from paper_2206_15117_b200 import Plan, ImagerError
+    params = CASES["wproj"]()
+    _, _, flat, _ = oracle_tables(params)
+    n = params["grid_size"]
+    with Plan(params, 100, user_tables=flat) as plan:
+        grid = torch.zeros((1, n, n), dtype=torch.complex64, device="cuda")
+        empty = lambda *s, dt=torch.float32: torch.zeros(s, dtype=dt, device="cuda")
+        plan.grid(empty(0, 3), empty(0, 1, dt=torch.complex64), empty(0, 1), grid)
+        plan.degrid(empty(0, 3), grid, empty(0, 1, dt=torch.complex64))
+        torch.cuda.synchronize()
+        assert torch.count_nonzero(grid).item() == 0
+        far = torch.full((100, 3), 1.0e7, dtype=torch.float32, device="cuda")       # every footprint leaves the grid
+        plan.grid(far, torch.ones((100, 1), dtype=torch.complex64, device="cuda"), torch.ones((100, 1), device="cuda"), grid)
+        out = torch.ones((100, 1), dtype=torch.complex64, device="cuda")
+        plan.degrid(far, grid, out)
+        torch.cuda.synchronize()
+        assert torch.count_nonzero(grid).item() == 0 and torch.count_nonzero(out).item() == 0
+        assert plan.info()["n_dropped"] == 100
+        with pytest.raises(ImagerError):
+            plan.grid(empty(101, 3), empty(101, 1, dt=torch.complex64), empty(101, 1), grid)   # TOO_MANY_VIS
+
+
+def test_adjointness_on_gpu(torch_cuda):
+    """<G v, g> = <v, G^H g> to 1e-6 relative (BASELINE.json north_star) on the CUDA path."""
+    torch = torch_cuda
+    from paper_2206_15117_b200 import Plan
+    for case in ("wproj", "awproj", "mosaic_even"):
+        params = CASES[case]()
+        nvis = 20000
+        uvw, vis, _, a = random_vis(params, nvis, seed=51, frac=0.3, a_planes=params["n_aplanes"] > 1)
+        _, _, flat, _ = oracle_tables(params)
+        n, npol, nc = params["grid_size"], params["n_pol"], params["n_corr"]
+        with Plan(params, nvis, user_tables=flat) as plan:
+            d_uvw, d_vis, _, d_a = _to_dev(torch, uvw, vis, None, a)
+            ones = torch.ones((nvis, nc), dtype=torch.float32, device="cuda")
+            gv = torch.zeros((npol, n, n), dtype=torch.complex64, device="cuda")
+            plan.grid(d_uvw, d_vis, ones, gv, d_a)
+            g = torch.randn((npol, n, n), dtype=torch.complex64, device="cuda")
+            hg = torch.zeros((nvis, nc), dtype=torch.complex64, device="cuda")
+            plan.degrid(d_uvw, g, hg, d_a, flags=1)
+            lhs = torch.vdot(g.to(torch.complex128).flatten(), gv.to(torch.complex128).flatten()).item()
+            rhs = torch.vdot(hg.to(torch.complex128).flatten(), d_vis.to(torch.complex128).flatten()).item()
+            assert abs(lhs - rhs) <= 1e-6 * abs(lhs), (case, lhs, rhs)

@@ -81,7 +81,7 @@ def test_bucket_sort_is_stable_and_partitions():
     rec = oidx.index_visibilities(uvw, a, params)
     assert rec["drop"].any() and not rec["drop"].all()
     keys = oidx.bucket_keys(rec, params, tile=32)
-    b = oidx.bucket_sort(keys, 4)
+    b = oidx.bucket_sort(keys, params, tile=32)
     perm = b["perm"]
     assert sorted(perm.tolist()) == list(range(nvis))
     sk = keys[perm]
@@ -89,10 +89,11 @@ def test_bucket_sort_is_stable_and_partitions():
     same = sk[1:] == sk[:-1]
     assert np.all(perm[1:][same] > perm[:-1][same])                 # stability
     assert b["n_kept"] == int((~rec["drop"]).sum())
-    # every bucket is one (kset, tile) pair
-    for i in range(len(b["bucket_id"])):
-        seg = perm[b["bucket_start"][i]:b["bucket_start"][i + 1]]
-        ks = rec["kset"][seg]
-        assert np.all(ks == ks[0])
-        assert np.all(rec["gx"][seg] // 32 == rec["gx"][seg][0] // 32)
-        assert np.all(rec["gy"][seg] // 32 == rec["gy"][seg][0] // 32)
+    off = b["bucket_offset"]
+    nt = 8
+    assert len(off) == 2 * 7 * nt * nt + 1 and off[0] == 0 and off[-1] == b["n_kept"]
+    for bucket in np.flatnonzero(np.diff(off))[:200]:               # every bucket is one (kset, tile) pair
+        seg = perm[off[bucket]:off[bucket + 1]]
+        assert np.all(rec["kset"][seg] == bucket // (nt * nt))
+        assert np.all(rec["gy"][seg] // 32 == (bucket // nt) % nt)
+        assert np.all(rec["gx"][seg] // 32 == bucket % nt)
