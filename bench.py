@@ -1,0 +1,318 @@
+#!/usr/bin/env python
+"""bench.py -- the contract benchmark: visibilities gridded + degridded per second on BASELINE.json's
+w-projection workload (configs[1], "config2": 36 antennas, 300 time steps x 64 channels = 12,096,000 visibilities,
+2048^2 grid, 32 w-planes, support 15..63, oversampling 4) on one B200.
+
+A "step" is one pass of the whole hot path over the batch: A1 index -> A2 bucket/sort -> A3 gridding -> A6 degridding
+(imager_grid cold + imager_degrid with index reuse).  `value` = visibilities / step time with inputs resident in HBM;
+`e2e` = the same through the C-ABI binding with HOST (pinned) buffers, H2D/D2H copies inside the timed region.
+`roofline` is for the dominant kernel (gridding, FP32-FMA bound): achieved = 8 flop x nominal complex MACs / its
+CUDA-event duration (warm call, index reused).  `cpu_baseline` = the oracle on a bounded sample of the same workload.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload config2] [--time-stride s]
+N > 1 runs N independent replicas (the path does not shard: BASELINE.json north_star "no sharding, no collectives").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+FP32_FMA_PER_CLK_SM = 128          # B200_PROFILING.md / SURVEY 8(d): 128 FP32 lanes per SM
+N_SM = 148
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        return json.load(open(path)), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+
+    def __init__(self, index=0):
+        super().__init__(daemon=True)
+        self.rows, self.stop_flag, self.index = [], False, index
+        self.query = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+                      "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+                      "clocks_event_reasons.sw_power_cap")
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.query}",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                parts = [p.strip() for p in out.strip().split(",")]
+                if len(parts) >= 7:
+                    self.rows.append(parts)
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        sm = sorted(float(r[0]) for r in self.rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(r[3 + i] == "Active" for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.rows[0][1]), "reasons": reasons,
+                "samples": len(self.rows), "power_w_max": max(float(r[2]) for r in self.rows)}
+
+
+def nominal_cmacs(params, rec):
+    """nominal complex MACs of one gridding pass = n_corr * n_pol * sum_k S_k^2 over kept visibilities."""
+    keep = ~rec["drop"]
+    return int(params["n_corr"]) * int(params["n_pol"]) * int(np.sum(rec["support"][keep].astype(np.int64) ** 2))
+
+
+def oracle_tables(params):
+    from oracle import kernels as okern
+    tabs, _ = okern.make_tables(params)
+    return okern.flatten_tables(tabs)
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle as it stands, on a bounded sample of the same workload."""
+    from oracle import index as oidx, gridder as ogrid
+    from synth import make_workload
+    ogrid.build()
+    stride = args.ref_time_stride
+    wl = make_workload(args.workload, time_stride=stride)
+    flat, offs = oracle_tables(wl.params)
+    n = wl.params["grid_size"]
+    times = []
+    for it in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        rec = oidx.index_visibilities(wl.uvw, wl.a_index, wl.params)
+        keys = oidx.bucket_keys(rec, wl.params, tile=32)
+        oidx.bucket_sort(keys, wl.params, tile=32)
+        out = ogrid.grid(rec, wl.vis, wl.weights, flat, offs, wl.params)
+        ogrid.degrid(rec, out["grid"].astype(np.complex64), flat, offs, wl.params)
+        if it >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    t = float(np.mean(times))
+    value = wl.nvis / t
+    cores = ogrid.max_threads()
+    sample = f"{args.workload} every {stride}th time step ({wl.nvis} visibilities, full grid and tables)"
+    line = {"metric": "visibilities gridded+degridded/sec", "value": value, "unit": "vis/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "impl": "reference",
+            "config": {"workload": args.workload, "nvis": wl.nvis, "grid": n, "sample": sample},
+            "cpu_baseline": {"value": value, "unit": "vis/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": "vis/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: libimager has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    from paper_2206_15117_b200 import Plan, REUSE_INDEX
+    from synth import make_workload
+    from oracle import index as oidx           # only for the nominal MAC count (integer bookkeeping) and cpu_baseline
+
+    wl = make_workload(args.workload, time_stride=args.time_stride)
+    params, nvis = wl.params, wl.nvis
+    n, nc, npol = params["grid_size"], params["n_corr"], params["n_pol"]
+    plan = Plan(params, nvis)                   # the library generates its own kernel tables (A0, untimed)
+    rec = oidx.index_visibilities(wl.uvw, wl.a_index, params)
+    cmacs = nominal_cmacs(params, rec)
+    del rec
+
+    # resident inputs
+    uvw = torch.from_numpy(wl.uvw).to(dev)
+    vis = torch.from_numpy(wl.vis).to(dev)
+    wts = torch.from_numpy(wl.weights).to(dev)
+    aidx = torch.from_numpy(wl.a_index).to(dev) if wl.a_index is not None else None
+    grid = torch.zeros((npol, n, n), dtype=torch.complex64, device=dev)
+    vout = torch.empty((nvis, nc), dtype=torch.complex64, device=dev)
+    stream = torch.cuda.current_stream()
+    launches = 0
+
+    def step():
+        nonlocal launches
+        grid.zero_()
+        plan.grid(uvw, vis, wts, grid, aidx)                      # cold: A1 + A2 + A3
+        launches += plan.last_launch_count()
+        plan.degrid(uvw, grid, vout, aidx, flags=REUSE_INDEX)     # A6
+        launches += plan.last_launch_count()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    launches = 0
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    for a, b in ev:
+        a.record(stream)
+        step()
+        b.record(stream)
+    barrier()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = float(sum(step_ms))
+    # dominant kernel: warm gridding and warm degridding calls timed on their own (index reused)
+    kern = {}
+    for name, fn in (("grid", lambda: plan.grid(uvw, vis, wts, grid, aidx, flags=REUSE_INDEX)),
+                     ("degrid", lambda: plan.degrid(uvw, grid, vout, aidx, flags=REUSE_INDEX))):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        es = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        for a, b in es:
+            a.record(stream)
+            fn()
+            b.record(stream)
+        torch.cuda.synchronize()
+        kern[name] = float(np.mean([a.elapsed_time(b) for a, b in es]))
+    barrier()
+    sampler.stop_flag = True
+
+    # end to end: pinned host buffers, H2D of the step's inputs and D2H of its results inside the timed region
+    h_uvw = torch.from_numpy(wl.uvw).pin_memory()
+    h_vis = torch.from_numpy(wl.vis).pin_memory()
+    h_wts = torch.from_numpy(wl.weights).pin_memory()
+    h_a = torch.from_numpy(wl.a_index).pin_memory() if wl.a_index is not None else None
+    h_out = torch.empty((nvis, nc), dtype=torch.complex64).pin_memory()
+    h_grid = torch.empty((npol, n, n), dtype=torch.complex64).pin_memory()
+
+    def e2e_step():
+        uvw.copy_(h_uvw, non_blocking=True)
+        vis.copy_(h_vis, non_blocking=True)
+        wts.copy_(h_wts, non_blocking=True)
+        if h_a is not None:
+            aidx.copy_(h_a, non_blocking=True)
+        step()
+        h_out.copy_(vout, non_blocking=True)
+        h_grid.copy_(grid, non_blocking=True)
+
+    e2e_steps = max(1, min(args.steps, 5))
+    e2e_step()
+    barrier()
+    t0 = torch.cuda.Event(enable_timing=True)
+    t1 = torch.cuda.Event(enable_timing=True)
+    t0.record(stream)
+    for _ in range(e2e_steps):
+        e2e_step()
+    t1.record(stream)
+    barrier()
+    e2e_ms = t0.elapsed_time(t1) / e2e_steps
+    h2d = h_uvw.numel() * 4 + h_vis.numel() * 8 + h_wts.numel() * 4 + (h_a.numel() * 4 if h_a is not None else 0)
+    d2h = h_out.numel() * 8 + h_grid.numel() * 8
+
+    times = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(times, op=dist.ReduceOp.MAX)
+    total_ms, e2e_ms = float(times[0]), float(times[1])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    peaks, peaks_kind = load_peaks()
+    ms_per_step = total_ms / args.steps
+    value = world * nvis / (ms_per_step * 1e-3)
+    peak_tflops = N_SM * FP32_FMA_PER_CLK_SM * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 * 2 / 1e12
+    achieved = 8.0 * cmacs / (kern["grid"] * 1e-3) / 1e12
+    traffic = None
+    prof = os.path.join(ROOT, "profiles", "traffic_bytes.json")
+    if os.path.exists(prof):
+        traffic = json.load(open(prof)).get("grid_kernel_dram_bytes_per_launch")
+    line = {
+        "metric": "visibilities gridded+degridded/sec", "value": value, "unit": "vis/s", "n_gpus": world,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": args.workload, "nvis": nvis, "grid": n, "n_wplanes": params["n_wplanes"],
+                   "support": [params["support_min"], params["support_max"]], "oversample": params["oversample"],
+                   "n_corr": nc, "time_stride": args.time_stride, "parallelism": f"replicas x{world}",
+                   "l2": "inputs (290 MB of visibilities + 33.5 MB grid) exceed the 126 MB L2; no explicit flush",
+                   "step": "imager_grid (index+sort+grid) + imager_degrid (index reused)"},
+        "clocks": sampler.summary(),
+        "e2e": {"value": world * nvis / (e2e_ms * 1e-3), "unit": "vis/s", "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms},
+        "gpu_launches": launches,
+        "roofline": {"bound": "alu", "kernel": "gridding (imager_grid, index reused)", "achieved": achieved,
+                     "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": traffic,
+                     "peak_kind": f"148 SM x 128 FP32 lanes x 2 flop x {peaks.get('sm_max_mhz', 1965.0):.0f} MHz "
+                                  f"({peaks_kind} max SM clock)",
+                     "kernel_ms": kern["grid"], "nominal_cmacs": cmacs,
+                     "grid_vis_per_s": nvis / (kern["grid"] * 1e-3), "grid_cmac_per_s": cmacs / (kern["grid"] * 1e-3),
+                     "degrid_ms": kern["degrid"], "degrid_vis_per_s": nvis / (kern["degrid"] * 1e-3),
+                     "degrid_frac": 8.0 * cmacs / (kern["degrid"] * 1e-3) / 1e12 / peak_tflops,
+                     "hbm_gbs_grid": (nvis * (16 + 4 + 8 * nc + 4 * nc) + 2 * npol * n * n * 8) / (kern["grid"] * 1e-3) / 1e9},
+        "step_ms_all": step_ms,
+    }
+    if not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(args)
+    print(json.dumps(line))
+    plan.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def cpu_baseline(args):
+    """The oracle as it stands on a bounded sample (about 10-30 s of CPU work) of the same workload."""
+    from oracle import index as oidx, gridder as ogrid
+    from synth import make_workload
+    stride = args.ref_time_stride
+    wl = make_workload(args.workload, time_stride=stride)
+    flat, offs = oracle_tables(wl.params)
+    t0 = time.perf_counter()
+    rec = oidx.index_visibilities(wl.uvw, wl.a_index, wl.params)
+    keys = oidx.bucket_keys(rec, wl.params, tile=32)
+    oidx.bucket_sort(keys, wl.params, tile=32)
+    out = ogrid.grid(rec, wl.vis, wl.weights, flat, offs, wl.params)
+    ogrid.degrid(rec, out["grid"].astype(np.complex64), flat, offs, wl.params)
+    t = time.perf_counter() - t0
+    return {"value": wl.nvis / t, "unit": "vis/s", "cores": ogrid.max_threads(), "kind": "oracle",
+            "sample": f"{args.workload} every {stride}th time step ({wl.nvis} visibilities, full grid and tables), "
+                      f"index+sort+grid+degrid in {t:.1f} s"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config2")
+    ap.add_argument("--time-stride", type=int, default=1, help="keep every n-th time step (1 = the full workload)")
+    ap.add_argument("--ref-time-stride", type=int, default=20, help="time-step stride of the CPU oracle's sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        if int(os.environ.get("RANK", "0")) == 0:
+            run_reference(args)
+        return
+    run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -139,6 +139,10 @@ int imager_debug_kernels(imager_plan* plan, int32_t kset, int32_t which, float* 
  * indexing (synchronises), [5] GPU kernel launches issued by the last imager_grid / imager_degrid call. */
 int imager_plan_info(imager_plan* plan, int64_t info_out[8]);
 
+/* Number of GPU kernels the last imager_grid / imager_degrid / imager_debug_index call on this plan launched
+ * (host-side counter, no synchronisation); negative status on a NULL plan. */
+int imager_last_launch_count(imager_plan* plan);
+
 /* Thread-local message of the last failing call on this thread ("" if none); valid until the next call. */
 const char* imager_last_error(void);
 

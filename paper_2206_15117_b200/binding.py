@@ -21,7 +21,7 @@ PATH_REFERENCE = 2
 
 EXPORTS = ("imager_plan_create", "imager_grid", "imager_degrid", "imager_plan_destroy",
            "imager_grid_image_transform", "imager_debug_index", "imager_debug_kernels", "imager_plan_info",
-           "imager_last_error")
+           "imager_last_launch_count", "imager_last_error")
 
 
 class ImagerError(RuntimeError):
@@ -59,6 +59,7 @@ def load_library() -> ctypes.CDLL:
                                        POINTER(c_int64), c_void_p]
     lib.imager_debug_kernels.argtypes = [c_void_p, c_int32, c_int32, c_void_p, POINTER(c_int32)]
     lib.imager_plan_info.argtypes = [c_void_p, POINTER(c_int64)]
+    lib.imager_last_launch_count.argtypes = [c_void_p]
     _lib = lib
     return lib
 
@@ -168,6 +169,9 @@ class Plan:
         import torch
         _check(load_library().imager_grid_image_transform(self._h, _dev_ptr(data, torch.complex64, "data"), direction,
                                                           float(norm), _stream_ptr(stream)), "imager_grid_image_transform")
+
+    def last_launch_count(self) -> int:
+        return int(load_library().imager_last_launch_count(self._h))
 
     # ---- debug exports --------------------------------------------------------------------------------------
     def info(self) -> dict:

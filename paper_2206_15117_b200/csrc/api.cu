@@ -245,6 +245,10 @@ extern "C" int imager_debug_kernels(imager_plan* plan, int32_t kset, int32_t whi
     return 0;
 }
 
+extern "C" int imager_last_launch_count(imager_plan* plan) {
+    return plan ? plan->last_launches : (int)IMAGER_ERR_INVALID_ARG;
+}
+
 extern "C" int imager_plan_info(imager_plan* plan, int64_t info_out[8]) {
     g_err[0] = 0;
     if (!plan || !info_out) { set_error("NULL argument"); return IMAGER_ERR_INVALID_ARG; }
