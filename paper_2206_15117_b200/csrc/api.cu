@@ -70,6 +70,7 @@ static void free_plan(imager_plan* pl) {
     cudaFree(pl->d_counters);
     cudaFree(pl->d_items);
     destroy_transform(pl);
+    tiled_release(pl);
     delete pl;
 }
 
@@ -186,7 +187,7 @@ extern "C" int imager_grid(imager_plan* plan, int64_t nvis, const float* uvw, co
     if (rc) return rc;
     if (!(flags & IMAGER_PATH_REFERENCE) && tiled_supported(plan))
         return launch_grid_tiled(plan, nvis, (const float2*)vis, weights, (float2*)grid, st);
-    return launch_grid_reference(plan, nvis, (const float2*)vis, weights, (float2*)grid, st);
+    return launch_grid_reference(plan, nvis, (const float2*)vis, weights, (float2*)grid, nullptr, st);
 }
 
 extern "C" int imager_degrid(imager_plan* plan, int64_t nvis, const float* uvw, const int32_t* a_index, const float* grid,
@@ -199,7 +200,7 @@ extern "C" int imager_degrid(imager_plan* plan, int64_t nvis, const float* uvw, 
     if (rc) return rc;
     if (!(flags & IMAGER_PATH_REFERENCE) && tiled_supported(plan))
         return launch_degrid_tiled(plan, nvis, (const float2*)grid, (float2*)vis_out, st);
-    return launch_degrid_reference(plan, nvis, (const float2*)grid, (float2*)vis_out, st);
+    return launch_degrid_reference(plan, nvis, (const float2*)grid, (float2*)vis_out, nullptr, st);
 }
 
 extern "C" int imager_grid_image_transform(imager_plan* plan, float* data, int32_t direction, double norm,

@@ -51,6 +51,8 @@ struct imager_plan {
     int32_t* d_counters = nullptr;       // [0] n_kept, [1] n_dropped, [2..] work-queue heads
     int64_t indexed_nvis = -1;
     bool index_valid = false;
+    int64_t index_epoch = 0;             // bumped by every re-indexing
+    void* tiled = nullptr;               // gridder_tiled.cu state (TiledState*)
 
     // tiled path work list
     int32_t* d_items = nullptr;          // [max_items][4]
@@ -69,9 +71,11 @@ namespace imager {
 int run_index_and_sort(imager_plan* pl, int64_t nvis, const float* uvw, const int32_t* a_index, cudaStream_t st);
 
 // gridder_ref.cu
+// set_mask (device, per kernel set, may be NULL): only visibilities of sets with a non-zero entry are processed
 int launch_grid_reference(imager_plan* pl, int64_t nvis, const float2* vis, const float* weights, float2* grid,
-                          cudaStream_t st);
-int launch_degrid_reference(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, cudaStream_t st);
+                          const int32_t* set_mask, cudaStream_t st);
+int launch_degrid_reference(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, const int32_t* set_mask,
+                            cudaStream_t st);
 int launch_sum_weights(imager_plan* pl, int64_t nvis, const float* weights, double* sum_weights, cudaStream_t st);
 
 // gridder_tiled.cu
@@ -79,6 +83,7 @@ bool tiled_supported(const imager_plan* pl);
 int launch_grid_tiled(imager_plan* pl, int64_t nvis, const float2* vis, const float* weights, float2* grid,
                       cudaStream_t st);
 int launch_degrid_tiled(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, cudaStream_t st);
+void tiled_release(imager_plan* pl);
 
 // tables.cu
 int build_tables(imager_plan* pl, const imager_params* user, cudaStream_t st);

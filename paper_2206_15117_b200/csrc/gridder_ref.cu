@@ -14,8 +14,8 @@ __global__ void __launch_bounds__(256)
 grid_ref_kernel(const int32_t* __restrict__ counters, const int32_t* __restrict__ perm,
                 const imager_record* __restrict__ rec, const float2* __restrict__ vis,
                 const float* __restrict__ weights, const float2* __restrict__ tab,
-                const int64_t* __restrict__ set_offset, const int32_t* __restrict__ set_support, int N, int O,
-                float2* __restrict__ grid) {
+                const int64_t* __restrict__ set_offset, const int32_t* __restrict__ set_support,
+                const int32_t* __restrict__ set_mask, int N, int O, float2* __restrict__ grid) {
     const int n_kept = counters[0];
     const int lane = threadIdx.x & 31;
     const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -23,6 +23,7 @@ grid_ref_kernel(const int32_t* __restrict__ counters, const int32_t* __restrict_
     for (int64_t i = warp0; i < n_kept; i += n_warps) {
         const int k = perm[i];
         const imager_record r = rec[k];
+        if (set_mask && !set_mask[r.kset]) continue;
         const int S = set_support[r.kset], h_lo = S / 2, SS = S * S;
         const int sub = (int)((r.sub >> 8) & 255u) * O + (int)(r.sub & 255u);
         float2 val[NC];
@@ -58,14 +59,15 @@ template <int NC, int NP>
 __global__ void __launch_bounds__(256)
 degrid_ref_kernel(int64_t nvis, const imager_record* __restrict__ rec, const int32_t* __restrict__ perm,
                   const float2* __restrict__ grid, const float2* __restrict__ tab,
-                  const int64_t* __restrict__ set_offset, const int32_t* __restrict__ set_support, int N, int O,
-                  float2* __restrict__ vis_out) {
+                  const int64_t* __restrict__ set_offset, const int32_t* __restrict__ set_support,
+                  const int32_t* __restrict__ set_mask, int N, int O, float2* __restrict__ vis_out) {
     const int lane = threadIdx.x & 31;
     const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int64_t n_warps = ((int64_t)gridDim.x * blockDim.x) >> 5;
     for (int64_t i = warp0; i < nvis; i += n_warps) {
         const int k = perm[i];                          // sorted order: dropped visibilities come last
         const imager_record r = rec[k];
+        if (set_mask && !set_mask[r.kset] && !((r.sub >> 16) & 1u)) continue;     // dropped ones are always written (0)
         float2 acc[NC];
 #pragma unroll
         for (int c = 0; c < NC; ++c) acc[c] = make_float2(0.f, 0.f);
@@ -137,31 +139,32 @@ int launch_sum_weights(imager_plan* pl, int64_t nvis, const float* weights, doub
 }
 
 int launch_grid_reference(imager_plan* pl, int64_t nvis, const float2* vis, const float* weights, float2* grid,
-                          cudaStream_t st) {
+                          const int32_t* set_mask, cudaStream_t st) {
     if (nvis == 0) return 0;
     const unsigned blocks = (unsigned)std::min<int64_t>((nvis + 7) / 8, 16 * kNumSMs);
     const int N = pl->p.grid_size, O = pl->p.oversample;
     if (pl->p.n_corr == 1)
         grid_ref_kernel<1, 1><<<blocks, 256, 0, st>>>(pl->d_counters, pl->d_perm[pl->sorted_buf], pl->d_rec, vis, weights,
-                                                      pl->d_tab_grid, pl->d_set_offset, pl->d_set_support, N, O, grid);
+                                                      pl->d_tab_grid, pl->d_set_offset, pl->d_set_support, set_mask, N, O, grid);
     else
         grid_ref_kernel<4, 4><<<blocks, 256, 0, st>>>(pl->d_counters, pl->d_perm[pl->sorted_buf], pl->d_rec, vis, weights,
-                                                      pl->d_tab_grid, pl->d_set_offset, pl->d_set_support, N, O, grid);
+                                                      pl->d_tab_grid, pl->d_set_offset, pl->d_set_support, set_mask, N, O, grid);
     pl->last_launches++;
     IMAGER_CUDA(cudaGetLastError());
     return 0;
 }
 
-int launch_degrid_reference(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, cudaStream_t st) {
+int launch_degrid_reference(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, const int32_t* set_mask,
+                            cudaStream_t st) {
     if (nvis == 0) return 0;
     const unsigned blocks = (unsigned)std::min<int64_t>((nvis + 7) / 8, 16 * kNumSMs);
     const int N = pl->p.grid_size, O = pl->p.oversample;
     if (pl->p.n_corr == 1)
         degrid_ref_kernel<1, 1><<<blocks, 256, 0, st>>>(nvis, pl->d_rec, pl->d_perm[pl->sorted_buf], grid, pl->d_tab_degrid,
-                                                        pl->d_set_offset, pl->d_set_support, N, O, vis_out);
+                                                        pl->d_set_offset, pl->d_set_support, set_mask, N, O, vis_out);
     else
         degrid_ref_kernel<4, 4><<<blocks, 256, 0, st>>>(nvis, pl->d_rec, pl->d_perm[pl->sorted_buf], grid, pl->d_tab_degrid,
-                                                        pl->d_set_offset, pl->d_set_support, N, O, vis_out);
+                                                        pl->d_set_offset, pl->d_set_support, set_mask, N, O, vis_out);
     pl->last_launches++;
     IMAGER_CUDA(cudaGetLastError());
     return 0;

@@ -207,6 +207,7 @@ int run_index_and_sort(imager_plan* pl, int64_t nvis, const float* uvw, const in
     IMAGER_CUDA(cudaGetLastError());
     pl->indexed_nvis = nvis;
     pl->index_valid = true;
+    pl->index_epoch++;
     return 0;
 }
 
