@@ -69,6 +69,8 @@ namespace imager {
 
 // index_sort.cu
 int run_index_and_sort(imager_plan* pl, int64_t nvis, const float* uvw, const int32_t* a_index, cudaStream_t st);
+// in-place exclusive scan of n int32; tmp needs sum over levels of (ceil(n/1024)+1) ints
+int exclusive_scan_i32(imager_plan* pl, int32_t* data, int64_t n, int32_t* tmp, cudaStream_t st);
 
 // gridder_ref.cu
 // set_mask (device, per kernel set, may be NULL): only visibilities of sets with a non-zero entry are processed

@@ -162,6 +162,10 @@ static int exclusive_scan(imager_plan* pl, int32_t* data, int64_t n, int32_t* tm
     return 0;
 }
 
+int exclusive_scan_i32(imager_plan* pl, int32_t* data, int64_t n, int32_t* tmp, cudaStream_t st) {
+    return exclusive_scan(pl, data, n, tmp, st);
+}
+
 __global__ void bucket_offset_kernel(const uint32_t* __restrict__ skey, int64_t n, int n_buckets, int oo,
                                      int32_t* __restrict__ bucket_offset, int32_t* __restrict__ counters) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
