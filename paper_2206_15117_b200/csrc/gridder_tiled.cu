@@ -1,44 +1,58 @@
-// gridder_tiled.cu -- the output-stationary ("tiled") gridding kernel (hot-path step A3) and its work planner.
+// gridder_tiled.cu -- the output-stationary ("tiled") gridding and degridding kernels (hot-path steps A3 / A6) and
+// their work planner.
 //
 // Why this shape: every complex MAC needs one 8-byte tap that no other MAC can share
-// (the tap index depends on visibility AND cell), so the shared-memory pipe (128 B/clk/SM; measured 4.59e12
-// LDS.64 lanes/s = 49 % of the FP32-FMA peak) is the binding unit, not HBM and not the FMA pipe.  The kernel
-//   (1) keeps grid cells in REGISTERS: a warp owns a 16 x 32 strip, its 8 x 4 lane block is replicated 2 x 8
-//       times (16 cells per lane, packed FFMA2 accumulators), so idle lanes only occur where a footprint edge
-//       cuts an 8 x 4 block;
-//   (2) keeps one "unit" (a kernel set, or a group of its sub-cell slices) resident in SHARED memory, rows
-//       zero-padded by 3 and pitched to 8 mod 16 taps so that LDS.64 of an 8 x 4 lane block is conflict-free;
-//   (3) streams bucket-sorted visibilities: 32 candidates per batch are tested against the strip by one lane
-//       each, the hits are compacted into per-warp descriptors in shared memory and replayed; a descriptor
-//       carries the precomputed tap address and the first/last active row group, so a hit costs one broadcast
-//       LDS.128 plus a Duff-style entry into the unrolled row-group chain (1 LDS.64 + 2 FFMA2 per group);
-//   (4) flushes a strip once per work entry with red.global.add.v2.f32.
-// Work planning (device side, at index time, cached while uvw is unchanged): entry = (unit, strip, part) with at
-// most kChunk candidate visibilities; blocks of kBlockEntries entries of one unit are pulled by persistent CTAs
-// from a global queue, the 16 warps of a CTA pull entries of the block from a shared counter.
+// (the tap index depends on visibility AND cell), and on sm_100a a warp-wide LDS.64 occupies the shared-memory
+// pipe for 2 clocks whatever its lane mask (measured), so the binding unit is LDS INSTRUCTIONS, not HBM and not
+// the FMA pipe (1 LDS.64 + 2 FFMA2 per 32 complex MACs = 49.6 % of the FP32 peak at best).  The kernels therefore
+//   (1) keep grid cells in REGISTERS: a warp owns a 16 x 32 strip, its 8 x 4 lane block replicated 2 x 8 times
+//       ("slots": 16 cells per lane, packed FFMA2 accumulators);
+//   (2) keep one unit (kernel set x group of sub-cell slices x Mueller element) resident in SHARED memory, rows
+//       zero-padded by 3, columns by 7, pitched to 8 mod 16 taps: an 8 x 4 lane block reads conflict-free, and
+//       lanes beyond a footprint edge read zeros without any per-lane test;
+//   (3) replay precomputed HITS: a hit is one (visibility, strip) pair with the tap address of the strip origin
+//       and the range of slots its footprint meets.  The hit lists are built on the device when (uvw, a_index)
+//       are indexed and are cached while those do not change (IMAGER_REUSE_INDEX: every major cycle after the
+//       first).  A hit costs one broadcast LDS.128, one REDUX for its warp-uniform slot range, and a jump into
+//       straight-line code specialised for that range (1 LDS.64 + 2 FFMA2 per slot, nothing else);
+//   (4) gridding flushes a strip once per work item with red.global.add.v2.f32; degridding loads the strip once
+//       per item, reduces each hit's 32 partial sums in batches of 8 by a shuffle transpose and adds the result to
+//       the visibility with one red.global.add.v2.f32.
+// Work planning: item = up to kItemHits hits of one (geometry unit, strip); block = consecutive items of one
+// geometry unit with about kBlockHits hits, times one Mueller element (s, c); persistent CTAs pull blocks from a
+// global queue, their 16 warps pull items of the block from a shared counter.
 #include "common.cuh"
 
 namespace imager {
 
 constexpr int kLaneW = 8, kLaneH = 4;                 // lane block
 constexpr int kNX = 2, kNY = 8;                       // replications: strip = 16 x 32 cells
-constexpr int kStripW = kLaneW * kNX, kStripH = kLaneH * kNY, kPad = kLaneH - 1;
+constexpr int kStripW = kLaneW * kNX, kStripH = kLaneH * kNY;
+constexpr int kPadY = kLaneH - 1, kPadX = kLaneW - 1;
 constexpr int kTiledThreads = 512, kWarps = kTiledThreads / 32;
-constexpr int kChunk = 512;                           // candidate visibilities per work entry
-constexpr int kBlockEntries = 64;                     // entries per CTA-level block
+constexpr int kItemHits = 128;                        // hits per work item (one flush / strip load each)
+constexpr int kBlockHits = 16384;                     // hits per CTA-level block
 constexpr int kStageBytes = kWarps * 32 * 16;         // per-warp hit descriptors
 constexpr int kMaxSmem = 227 * 1024;
-constexpr int64_t kMaxPlanCells = 48 << 20;           // (unit, strip) pairs the planner may enumerate
+constexpr int kTableBudget = kMaxSmem - kStageBytes - 1024;
+constexpr int64_t kMaxPlanCells = 48 << 20;           // (geometry unit, strip) pairs the planner may enumerate
+constexpr uint32_t kTapBias = 1u << 20;
 
 struct SetPlan {           // per kernel set (host-built)
-    int32_t pitch;         // taps per padded row, = 8 mod 16
-    int32_t group_slices;  // sub-cell slices resident at once (O*O, O or 1); 0 = not tiled (reference path)
+    int32_t pitch;         // taps per padded row, = 8 mod 16, >= S + 2 kPadX
+    int32_t rows;          // S + 2 kPadY
+    int32_t group_slices;  // sub-cell slices resident at once (a power of two <= O*O)
     int32_t n_groups;
-    int32_t unit_base;     // first unit of this set; unit = unit_base + group
+    int32_t gu_base;       // first geometry unit of this set; gu = gu_base + group
+    int32_t pad[3];
 };
 
-struct Entry { int32_t unit, strip, part, pad; };
-struct Block { int32_t kset, group, first, count; };
+struct Item { int32_t strip, hit_begin, hit_count, pad; };
+struct Block { int32_t gu, sc, item_begin, item_count; };
+
+struct Geometry {
+    int N, O, nt, strips_per_row, n_strips, n_sets, n_gu, n_pol, n_corr;
+};
 
 __device__ __forceinline__ void ffma2(float2& d, const float2 a, const float2 b) {
     unsigned long long dd = *reinterpret_cast<unsigned long long*>(&d);
@@ -50,7 +64,7 @@ __device__ __forceinline__ void ffma2(float2& d, const float2 a, const float2 b)
 
 __device__ __forceinline__ float2 lds64(uint32_t addr) {
     float2 v;
-    asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
     return v;
 }
 
@@ -81,9 +95,17 @@ __global__ void gather_values_kernel(const int32_t* __restrict__ counters, const
     }
 }
 
-struct Geometry {
-    int N, O, nt, strips_per_row, n_strips, n_sets, n_units;
-};
+// degridding epilogue: sorted-order sums -> vis_out in input order (dropped visibilities predict 0)
+template <int NC>
+__global__ void scatter_values_kernel(int64_t nvis, const int32_t* __restrict__ counters, const int32_t* __restrict__ perm,
+                                      const float2* __restrict__ sval, float2* __restrict__ vis_out) {
+    const int n_kept = counters[0];
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvis; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t k = perm[i];
+#pragma unroll
+        for (int c = 0; c < NC; ++c) vis_out[k * NC + c] = i < n_kept ? sval[i * NC + c] : make_float2(0.f, 0.f);
+    }
+}
 
 // candidate visibilities of (kset, strip): the bucket rows / columns whose footprints can reach the strip
 __device__ __forceinline__ void strip_buckets(const Geometry& g, int strip, int S, int& Xw, int& Yw, int& bx_lo, int& bx_hi,
@@ -99,136 +121,306 @@ __device__ __forceinline__ void strip_buckets(const Geometry& g, int strip, int 
 }
 
 // ---- planner ---------------------------------------------------------------------------------------------
-// parts[unit * n_strips + strip] = ceil(candidates / kChunk)
-__global__ void plan_count_kernel(const Geometry g, const SetPlan* __restrict__ set_plan, const int32_t* __restrict__ unit_set,
-                                  const int32_t* __restrict__ set_support, const int32_t* __restrict__ bucket_offset,
-                                  int32_t* __restrict__ parts) {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i > (int64_t)g.n_units * g.n_strips) return;
-    if (i == (int64_t)g.n_units * g.n_strips) { parts[i] = 0; return; }
-    const int unit = (int)(i / g.n_strips), strip = (int)(i - (int64_t)unit * g.n_strips);
-    const int kset = unit_set[unit];
-    int Xw, Yw, bx_lo, bx_hi, by_lo, by_hi;
-    strip_buckets(g, strip, set_support[kset], Xw, Yw, bx_lo, bx_hi, by_lo, by_hi);
-    int c = 0;
-    for (int by = by_lo; by <= by_hi; ++by) {
-        const int b0 = (kset * g.nt + by) * g.nt;
-        c += bucket_offset[b0 + bx_hi + 1] - bucket_offset[b0 + bx_lo];
+// A hit of (gu, strip): a kept visibility of the unit's kernel set whose sub-cell slice is in the unit's group and
+// whose footprint meets the strip.  Record: .x = sorted index of the visibility,
+// .y = (tap offset of the strip origin within the group's shared-memory image + kTapBias) | ctrl << 24,
+// ctrl = jl | (jh - 1) << 3 | halves << 6: slots jl .. jh-1 of x-half 0 (bit 6) and / or 1 (bit 7).
+struct PlanArgs {
+    Geometry g;
+    const SetPlan* set_plan;
+    const int32_t* gu_set;
+    const int32_t* set_support;
+    const int32_t* bucket_offset;
+    const uint2* sgeo;
+};
+
+// ctrl byte of a candidate against a strip, or 0 if it is no hit (a hit always has bit 6 or 7 set)
+__device__ __forceinline__ uint32_t hit_ctrl(int dx0, int dy0, int S, int sub, int group_slices) {
+    const bool hit = (dx0 + kStripW > 0) && (dx0 < S) && (dy0 + kStripH > 0) && (dy0 < S) &&
+                     ((unsigned)sub < (unsigned)group_slices);
+    if (!hit) return 0u;
+    const int jl = (dy0 + kPadY < 0) ? (-dy0) / kLaneH : 0;        // first slot reaching row 0
+    const int jh = min(kNY, (S - 1 - dy0) / kLaneH + 1);           // one past the last slot
+    const uint32_t left = (dx0 + kLaneW > 0) ? 1u : 0u;            // x-half 0 meets the footprint
+    const uint32_t right = (dx0 + kLaneW < S) ? 1u : 0u;           // x-half 1 meets the footprint
+    return (uint32_t)jl | ((uint32_t)(jh - 1) << 3) | (left << 6) | (right << 7);
+}
+
+// dense variant number of a ctrl byte (108 values)
+#define IMAGER_VARIANT(H, JL, JH1) (((H) - 1) * 36 + (JL) * 8 - ((JL) * ((JL) - 1)) / 2 + (JH1) - (JL))
+constexpr int kVariants = 108;
+
+__device__ __forceinline__ uint32_t ctrl_variant(uint32_t ctrl) {
+    const int jl = (int)(ctrl & 7u), jh1 = (int)((ctrl >> 3) & 7u), h = (int)(ctrl >> 6);
+    return (uint32_t)IMAGER_VARIANT(h, jl, jh1);
+}
+
+// MODE 0: count hits (hits[cell], items[cell]); MODE 1: write hit records, SORTED BY VARIANT within the cell (stable:
+// candidate order is kept within a variant, so the result is deterministic), and the items.  One warp per (gu, strip).
+template <int MODE>
+__global__ void __launch_bounds__(256) plan_hits_kernel(const PlanArgs a, int32_t* __restrict__ hits, int32_t* __restrict__ items,
+                                                        uint2* __restrict__ hit_rec, Item* __restrict__ item_rec) {
+    __shared__ int32_t s_bin[8][128];
+    const Geometry& g = a.g;
+    const int64_t cell = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int64_t n_cells = (int64_t)g.n_gu * g.n_strips;
+    const int lane = threadIdx.x & 31, warp = (threadIdx.x >> 5) & 7;
+    if (cell > n_cells) return;
+    if (cell == n_cells) {                                   // terminator of the exclusive scans
+        if (MODE == 0 && lane == 0) hits[cell] = items[cell] = 0;
+        return;
     }
-    parts[i] = (c + kChunk - 1) / kChunk;
+    const int gu = (int)(cell / g.n_strips), strip = (int)(cell - (int64_t)gu * g.n_strips);
+    const int kset = a.gu_set[gu];
+    const SetPlan sp = a.set_plan[kset];
+    const int S = a.set_support[kset], h_lo = S / 2;
+    const int sub_lo = (gu - sp.gu_base) * sp.group_slices;
+    int Xw, Yw, bx_lo, bx_hi, by_lo, by_hi;
+    strip_buckets(g, strip, S, Xw, Yw, bx_lo, bx_hi, by_lo, by_hi);
+    int out = 0;
+    if (MODE == 1) {
+        out = hits[cell];
+        const int n_hits = hits[cell + 1] - out;
+        if (n_hits == 0) return;
+        const int i0 = items[cell], n_items = items[cell + 1] - i0;
+        for (int p = lane; p < n_items; p += 32)
+            item_rec[i0 + p] = Item{strip, out + p * kItemHits, min(kItemHits, n_hits - p * kItemHits), gu};
+        for (int v = lane; v < 128; v += 32) s_bin[warp][v] = 0;
+        __syncwarp();
+    }
+    const int slice_taps = sp.rows * sp.pitch;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    int count = 0;
+    // pass 0: count (MODE 0) or histogram by variant (MODE 1); pass 1 (MODE 1 only): stable scatter
+    for (int pass = 0; pass <= MODE; ++pass) {
+        if (pass == 1) {                                     // exclusive prefix of the 108 bins, 4 per lane
+            __syncwarp();
+            int c[4], t = 0;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                c[q] = s_bin[warp][4 * lane + q];
+                t += c[q];
+            }
+            int inc = t;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, inc, d);
+                if (lane >= d) inc += y;
+            }
+            int run = inc - t;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                s_bin[warp][4 * lane + q] = run;
+                run += c[q];
+            }
+            __syncwarp();
+        }
+        for (int by = by_lo; by <= by_hi; ++by) {
+            const int b0 = (kset * g.nt + by) * g.nt;
+            const int r0 = a.bucket_offset[b0 + bx_lo], r1 = a.bucket_offset[b0 + bx_hi + 1];
+            for (int i0 = r0; i0 < r1; i0 += 32) {
+                const int idx = i0 + lane;
+                uint32_t ctrl = 0u;
+                int dx0 = 0, dy0 = 0, sub = 0;
+                if (idx < r1) {
+                    const uint2 geo = a.sgeo[idx];
+                    const int gx = (int)(geo.x & 0xffffu), gy = (int)(geo.x >> 16);
+                    dx0 = Xw - (gx - h_lo);                                  // tap coordinates of the strip origin
+                    dy0 = Yw - (gy - h_lo);
+                    sub = (int)geo.y - sub_lo;
+                    ctrl = hit_ctrl(dx0, dy0, S, sub, sp.group_slices);
+                }
+                const unsigned m = __ballot_sync(0xffffffffu, ctrl != 0u);
+                if (MODE == 0) {
+                    count += __popc(m);
+                } else if (m) {
+                    const uint32_t v = ctrl ? ctrl_variant(ctrl) : 127u;
+                    if (pass == 0) {
+                        if (ctrl) atomicAdd(&s_bin[warp][v], 1);
+                    } else {
+                        const unsigned peers = __match_any_sync(0xffffffffu, v);
+                        const int leader = __ffs(peers) - 1, rank = __popc(peers & lt_mask);
+                        int base = 0;
+                        if (lane == leader && ctrl) {
+                            base = s_bin[warp][v];
+                            s_bin[warp][v] = base + __popc(peers);
+                        }
+                        base = __shfl_sync(0xffffffffu, base, leader);
+                        if (ctrl) {
+                            const int tapoff = sub * slice_taps + (dy0 + kPadY) * sp.pitch + dx0 + kPadX;
+                            hit_rec[out + base + rank] = make_uint2((uint32_t)idx, (uint32_t)(tapoff + (int)kTapBias) | (ctrl << 24));
+                        }
+                    }
+                }
+            }
+        }
+    }
+    if (MODE == 0 && lane == 0) {
+        hits[cell] = count;
+        items[cell] = (count + kItemHits - 1) / kItemHits;
+    }
 }
 
-__global__ void plan_fill_kernel(const Geometry g, const int32_t* __restrict__ entry_start, Entry* __restrict__ entries) {
-    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= (int64_t)g.n_units * g.n_strips) return;
-    const int unit = (int)(i / g.n_strips), strip = (int)(i - (int64_t)unit * g.n_strips);
-    const int e0 = entry_start[i], e1 = entry_start[i + 1];
-    for (int e = e0; e < e1; ++e) entries[e] = Entry{unit, strip, e - e0, 0};
-}
-
-// one thread block: blocks of at most kBlockEntries entries, never spanning two units
-__global__ void plan_blocks_kernel(const Geometry g, const SetPlan* __restrict__ set_plan, const int32_t* __restrict__ unit_set,
-                                   const int32_t* __restrict__ entry_start, Block* __restrict__ blocks,
-                                   int32_t* __restrict__ n_blocks) {
+// one thread block: per geometry unit, blocks of about kBlockHits hits (whole items), replicated for every Mueller
+// element sc = s * n_corr + c.  Block order is irrelevant (a work queue consumes them).
+__global__ void plan_blocks_kernel(const Geometry g, const int32_t* __restrict__ hit_start, const int32_t* __restrict__ item_start,
+                                   const Item* __restrict__ item_rec, Block* __restrict__ blocks, int32_t* __restrict__ n_blocks,
+                                   int max_blocks) {
     __shared__ int s_total;
     if (threadIdx.x == 0) s_total = 0;
     __syncthreads();
-    for (int u0 = 0; u0 < g.n_units; u0 += blockDim.x) {
-        const int u = u0 + threadIdx.x;
-        int first = 0, cnt = 0;
-        if (u < g.n_units) {
-            first = entry_start[(int64_t)u * g.n_strips];
-            cnt = entry_start[(int64_t)(u + 1) * g.n_strips] - first;
+    const int n_sc = g.n_pol * g.n_corr;
+    for (int gu = threadIdx.x; gu < g.n_gu; gu += blockDim.x) {
+        const int64_t c0 = (int64_t)gu * g.n_strips, c1 = c0 + g.n_strips;
+        const int h0 = hit_start[c0], h1 = hit_start[c1], i0 = item_start[c0], i1 = item_start[c1];
+        if (h1 == h0) continue;
+        const int nb = (h1 - h0 + kBlockHits - 1) / kBlockHits;
+        const int base = atomicAdd(&s_total, nb * n_sc);
+        if (base + nb * n_sc > max_blocks) continue;                      // cannot happen: max_blocks is an upper bound
+        int first = i0;
+        for (int b = 0; b < nb; ++b) {
+            // first item whose hit_begin >= h0 + (b + 1) * kBlockHits
+            const int limit = h0 + (b + 1) * kBlockHits;
+            int lo = first, hi = i1;
+            while (lo < hi) {
+                const int mid = (lo + hi) >> 1;
+                if (item_rec[mid].hit_begin < limit) lo = mid + 1; else hi = mid;
+            }
+            const int last = (b == nb - 1) ? i1 : lo;
+            for (int sc = 0; sc < n_sc; ++sc) blocks[base + sc * nb + b] = Block{gu, sc, first, last - first};
+            first = last;
         }
-        const int nb = (cnt + kBlockEntries - 1) / kBlockEntries;
-        const int base = nb ? atomicAdd(&s_total, nb) : 0;            // block order is irrelevant
-        if (nb) {
-            const int kset = unit_set[u];
-            for (int b = 0; b < nb; ++b)
-                blocks[base + b] = Block{kset, u - set_plan[kset].unit_base, first + b * kBlockEntries,
-                                         min(kBlockEntries, cnt - b * kBlockEntries)};
-        }
-        __syncthreads();
     }
-    if (threadIdx.x == 0) *n_blocks = s_total;
+    __syncthreads();
+    if (threadIdx.x == 0) *n_blocks = min(s_total, max_blocks);
 }
 
-// ---- the gridding kernel ---------------------------------------------------------------------------------
+// ---- the kernels -----------------------------------------------------------------------------------------
 struct TiledArgs {
     Geometry g;
-    const int32_t* bucket_offset;
-    const uint2* sgeo;
-    const float2* sval;
+    const uint2* hit_rec;
+    const Item* items;
+    const Block* blocks;
+    const int32_t* n_blocks;
+    int32_t* queue;
     const float2* tab;
     const int64_t* set_offset;
     const int32_t* set_support;
     const SetPlan* set_plan;
-    const Entry* entries;
-    const Block* blocks;
-    const int32_t* n_blocks;
-    int32_t* queue;
+    const int32_t* gu_set;
 };
 
-// copy one slice group of kernel set `kset` into shared memory: [slice][row -3 .. S+2][pitch], zero padded
-__device__ void load_table_group(const TiledArgs& a, int kset, int group, const SetPlan sp, int S, float2* tab_s) {
-    const float2* T = a.tab + a.set_offset[kset];
-    const int rows = S + 2 * kPad;
-    const int per_slice = rows * sp.pitch;
+// copy one slice group of element sc of kernel set `kset` into shared memory: [slice][row -3 .. S+2][col -7 ..], zero padded
+__device__ void load_table_group(const TiledArgs& a, int kset, int group, int sc, const SetPlan sp, int S, float2* tab_s) {
+    const int OO = a.g.O * a.g.O;
+    const float2* T = a.tab + a.set_offset[kset] + ((int64_t)sc * OO + (int64_t)group * sp.group_slices) * S * S;
+    const int per_slice = sp.rows * sp.pitch;
     const int total = sp.group_slices * per_slice;
     for (int i = threadIdx.x; i < total; i += blockDim.x) {
         const int sl = i / per_slice, rem = i - sl * per_slice;
-        const int r = rem / sp.pitch, row = r - kPad, col = rem - r * sp.pitch;
+        const int r = rem / sp.pitch, row = r - kPadY, col = rem - r * sp.pitch - kPadX;
         float2 v = make_float2(0.f, 0.f);
-        if (row >= 0 && row < S && col < S) v = __ldg(&T[((int64_t)(group * sp.group_slices + sl) * S + row) * S + col]);
+        if (row >= 0 && row < S && col >= 0 && col < S) v = __ldg(&T[((int64_t)sl * S + row) * S + col]);
         tab_s[i] = v;
     }
 }
 
-// one row group: tap loads for the two 8-column halves of the strip, 2 FFMA2 each (A += t*vr, B += t*vi)
-#define IMAGER_SLOT_BOTH(j)                                \
-    {                                                      \
-        const float2 t0 = lds64(addr0 + (j) * step0);      \
-        const float2 t1 = lds64(addr1 + (j) * step1);      \
-        ffma2(A0[j], t0, vrr);                             \
-        ffma2(B0[j], t0, vii);                             \
-        ffma2(A1[j], t1, vrr);                             \
-        ffma2(B1[j], t1, vii);                             \
+// ---- gridding bodies: a run of `cnt` staged hits with the same slot range, straight-line code per hit -----------
+// slot j, x-half h: tap at addr + j * step + 64 h; A += t * vr, B += t * vi  (re = A.x - B.y, im = A.y + B.x at the flush)
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+    uint4 d;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(d.x), "=r"(d.y), "=r"(d.z), "=r"(d.w) : "r"(addr));
+    return d;
+}
+
+template <int H, int JL, int JH>
+__device__ __forceinline__ void grid_run(float2 (&A0)[kNY], float2 (&B0)[kNY], float2 (&A1)[kNY], float2 (&B1)[kNY],
+                                         uint32_t desc_addr, int cnt, const uint32_t lane_off, const uint32_t step) {
+    uint4 d = lds128(desc_addr);
+#pragma unroll 1
+    for (int i = 0; i < cnt; ++i) {
+        desc_addr += 16;
+        const uint4 dn = lds128(desc_addr);                  // next descriptor (one past the run at its end: unused)
+        const uint32_t addr = d.x + lane_off;
+        const float vr = __uint_as_float(d.y), vi = __uint_as_float(d.z);
+        const float2 vrr = make_float2(vr, vr), vii = make_float2(vi, vi);
+        // at most 8 tap loads in flight: chunks of 4 slots (both halves) or 8 slots (one half)
+        constexpr int kChunk = (H == 3) ? 4 : 8;
+#pragma unroll
+        for (int j0 = JL; j0 < JH; j0 += kChunk) {
+            float2 t0[kChunk], t1[kChunk];
+#pragma unroll
+            for (int j = j0; j < j0 + kChunk && j < JH; ++j) {
+                if (H & 1) t0[j - j0] = lds64(addr + j * step);
+                if (H & 2) t1[j - j0] = lds64(addr + j * step + kLaneW * 8);
+            }
+#pragma unroll
+            for (int j = j0; j < j0 + kChunk && j < JH; ++j) {
+                if (H & 1) {
+                    ffma2(A0[j], t0[j - j0], vrr);
+                    ffma2(B0[j], t0[j - j0], vii);
+                }
+                if (H & 2) {
+                    ffma2(A1[j], t1[j - j0], vrr);
+                    ffma2(B1[j], t1[j - j0], vii);
+                }
+            }
+        }
+        d = dn;
     }
-#define IMAGER_SLOT_LEFT(j)                                \
-    {                                                      \
-        const float2 t0 = lds64(addr0 + (j) * step0);      \
-        ffma2(A0[j], t0, vrr);                             \
-        ffma2(B0[j], t0, vii);                             \
-    }
-#define IMAGER_SLOT_RIGHT(j)                               \
-    {                                                      \
-        const float2 t1 = lds64(addr1 + (j) * step1);      \
-        ffma2(A1[j], t1, vrr);                             \
-        ffma2(B1[j], t1, vii);                             \
-    }
-// enter the unrolled row-group chain at jl, leave after jh - 1 (jl, jh are warp-uniform: they come from a REDUX)
-#define IMAGER_CHAIN(SLOT)                         \
-    switch (jl) {                                  \
-        case 0: SLOT(0) if (jh == 1) break;        \
-        case 1: SLOT(1) if (jh == 2) break;        \
-        case 2: SLOT(2) if (jh == 3) break;        \
-        case 3: SLOT(3) if (jh == 4) break;        \
-        case 4: SLOT(4) if (jh == 5) break;        \
-        case 5: SLOT(5) if (jh == 6) break;        \
-        case 6: SLOT(6) if (jh == 7) break;        \
-        case 7: SLOT(7)                            \
+}
+
+#define IMAGER_CASE(FN, H, JL, JH1) \
+    case IMAGER_VARIANT(H, JL, JH1): FN<H, JL, (JH1) + 1> IMAGER_BODY_ARGS; break;
+#define IMAGER_CASES_H(FN, H)                                                                                           \
+    IMAGER_CASE(FN, H, 0, 0) IMAGER_CASE(FN, H, 0, 1) IMAGER_CASE(FN, H, 0, 2) IMAGER_CASE(FN, H, 0, 3)                  \
+    IMAGER_CASE(FN, H, 0, 4) IMAGER_CASE(FN, H, 0, 5) IMAGER_CASE(FN, H, 0, 6) IMAGER_CASE(FN, H, 0, 7)                  \
+    IMAGER_CASE(FN, H, 1, 1) IMAGER_CASE(FN, H, 1, 2) IMAGER_CASE(FN, H, 1, 3) IMAGER_CASE(FN, H, 1, 4)                  \
+    IMAGER_CASE(FN, H, 1, 5) IMAGER_CASE(FN, H, 1, 6) IMAGER_CASE(FN, H, 1, 7)                                           \
+    IMAGER_CASE(FN, H, 2, 2) IMAGER_CASE(FN, H, 2, 3) IMAGER_CASE(FN, H, 2, 4) IMAGER_CASE(FN, H, 2, 5)                  \
+    IMAGER_CASE(FN, H, 2, 6) IMAGER_CASE(FN, H, 2, 7)                                                                    \
+    IMAGER_CASE(FN, H, 3, 3) IMAGER_CASE(FN, H, 3, 4) IMAGER_CASE(FN, H, 3, 5) IMAGER_CASE(FN, H, 3, 6)                  \
+    IMAGER_CASE(FN, H, 3, 7)                                                                                             \
+    IMAGER_CASE(FN, H, 4, 4) IMAGER_CASE(FN, H, 4, 5) IMAGER_CASE(FN, H, 4, 6) IMAGER_CASE(FN, H, 4, 7)                  \
+    IMAGER_CASE(FN, H, 5, 5) IMAGER_CASE(FN, H, 5, 6) IMAGER_CASE(FN, H, 5, 7)                                           \
+    IMAGER_CASE(FN, H, 6, 6) IMAGER_CASE(FN, H, 6, 7)                                                                    \
+    IMAGER_CASE(FN, H, 7, 7)
+#define IMAGER_DISPATCH(FN, variant)   \
+    switch (variant) {                 \
+        IMAGER_CASES_H(FN, 1)          \
+        IMAGER_CASES_H(FN, 2)          \
+        IMAGER_CASES_H(FN, 3)          \
+        default: break;                \
     }
 
-__global__ void __launch_bounds__(kTiledThreads, 1) grid_tiled_kernel(const TiledArgs a, float2* __restrict__ grid) {
+// slot mask of a ctrl byte: bits 0-7 x-half 0, bits 8-15 x-half 1
+__device__ __forceinline__ uint32_t ctrl_slot_mask(uint32_t ctrl) {
+    const uint32_t jl = ctrl & 7u, jh = ((ctrl >> 3) & 7u) + 1u;
+    const uint32_t rows = (1u << jh) - (1u << jl);
+    return ((ctrl & 0x40u) ? rows : 0u) | ((ctrl & 0x80u) ? rows << 8 : 0u);
+}
+
+// Shared by gridding and degridding: block / item queues and the staging of hit descriptors.
+// stage[lane] = {shared address of the strip-origin tap, value.x, value.y, sorted index}
+struct WarpCtx {
+    uint4* stage;
+    uint32_t tab_addr;
+    int lane, lx, ly;
+};
+
+template <int NC>
+__global__ void __launch_bounds__(kTiledThreads, 1)
+grid_tiled_kernel(const TiledArgs a, const float2* __restrict__ sval, float2* __restrict__ grid) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     uint4* stage = reinterpret_cast<uint4*>(smem_raw) + (threadIdx.x >> 5) * 32;       // this warp's descriptors
     float2* tab_s = reinterpret_cast<float2*>(smem_raw + kStageBytes);
     const uint32_t tab_addr = (uint32_t)__cvta_generic_to_shared(tab_s);
+    const uint32_t stage_addr = (uint32_t)__cvta_generic_to_shared(stage);
     __shared__ int s_block, s_next;
     const int lane = threadIdx.x & 31, lx = lane & (kLaneW - 1), ly = lane >> 3;
     const Geometry g = a.g;
     const int n_blocks = *a.n_blocks;
-    int cur_kset = -1, cur_group = -1;
+    int cur_gu = -1, cur_sc = -1;
     for (;;) {
         __syncthreads();                                   // everyone is done with the previous block
         if (threadIdx.x == 0) {
@@ -238,103 +430,71 @@ __global__ void __launch_bounds__(kTiledThreads, 1) grid_tiled_kernel(const Tile
         __syncthreads();
         if (s_block >= n_blocks) break;
         const Block blk = a.blocks[s_block];
-        const SetPlan sp = a.set_plan[blk.kset];
-        const int S = a.set_support[blk.kset], h_lo = S / 2;
-        if (blk.kset != cur_kset || blk.group != cur_group) {
-            load_table_group(a, blk.kset, blk.group, sp, S, tab_s);
-            cur_kset = blk.kset;
-            cur_group = blk.group;
+        const int kset = a.gu_set[blk.gu];
+        const SetPlan sp = a.set_plan[kset];
+        const int S = a.set_support[kset];
+        if (blk.gu != cur_gu || blk.sc != cur_sc) {
+            load_table_group(a, kset, blk.gu - sp.gu_base, blk.sc, sp, S, tab_s);
+            cur_gu = blk.gu;
+            cur_sc = blk.sc;
             __syncthreads();
         }
-        const int slice_bytes = (S + 2 * kPad) * sp.pitch * 8;
-        const int step_bytes = kLaneH * sp.pitch * 8;              // one row group down
-        const int sub_lo = blk.group * sp.group_slices;
+        const int s_pol = blk.sc / g.n_corr, c_corr = blk.sc - s_pol * g.n_corr;
+        float2* gplane = grid + (int64_t)s_pol * g.N * g.N;
+        const uint32_t step = (uint32_t)(kLaneH * sp.pitch * 8);              // one slot down
         const uint32_t lane_off = (uint32_t)((ly * sp.pitch + lx) * 8);
         for (;;) {
-            int ei = 0;
-            if (lane == 0) ei = atomicAdd(&s_next, 1);
-            ei = __shfl_sync(0xffffffffu, ei, 0);
-            if (ei >= blk.count) break;
-            const Entry ent = a.entries[blk.first + ei];
-            int Xw, Yw, bx_lo, bx_hi, by_lo, by_hi;
-            strip_buckets(g, ent.strip, S, Xw, Yw, bx_lo, bx_hi, by_lo, by_hi);
+            int ii = 0;
+            if (lane == 0) ii = atomicAdd(&s_next, 1);
+            ii = __shfl_sync(0xffffffffu, ii, 0);
+            if (ii >= blk.item_count) break;
+            const Item it = a.items[blk.item_begin + ii];
             float2 A0[kNY], B0[kNY], A1[kNY], B1[kNY];
 #pragma unroll
             for (int j = 0; j < kNY; ++j) A0[j] = B0[j] = A1[j] = B1[j] = make_float2(0.f, 0.f);
-            bool any = false;
-            int skip = ent.part * kChunk, take = kChunk;
-            for (int by = by_lo; by <= by_hi && take > 0; ++by) {
-                const int b0 = (blk.kset * g.nt + by) * g.nt;
-                const int r0 = a.bucket_offset[b0 + bx_lo], r1 = a.bucket_offset[b0 + bx_hi + 1];
-                if (skip >= r1 - r0) { skip -= r1 - r0; continue; }
-                const int beg = r0 + skip, end = min(r1, beg + take);
-                skip = 0;
-                take -= end - beg;
-                for (int i0 = beg; i0 < end; i0 += 32) {
-                    const int idx = i0 + lane;
-                    bool hit = false;
-                    uint32_t packed = 0u;
-                    if (idx < end) {
-                        const uint2 geo = a.sgeo[idx];
-                        const int gx = (int)(geo.x & 0xffffu), gy = (int)(geo.x >> 16);
-                        const int dx0 = Xw - (gx - h_lo), dy0 = Yw - (gy - h_lo);   // tap coordinates of the strip origin
-                        const int sub = (int)geo.y - sub_lo;
-                        hit = (dx0 + kStripW > 0) && (dx0 < S) && (dy0 + kStripH > 0) && (dy0 < S) &&
-                              ((unsigned)sub < (unsigned)sp.group_slices);
-                        if (hit) {
-                            const float2 v = a.sval[idx];
-                            const int jl = (dy0 + kPad < 0) ? (-dy0) / kLaneH : 0;        // first group reaching row 0
-                            const int jh = min(kNY, (S - 1 - dy0) / kLaneH + 1);          // one past the last group
-                            const uint32_t left = (dx0 + kLaneW > 0) ? 1u : 0u;           // x-half 0 meets the footprint
-                            const uint32_t right = (dx0 + kLaneW < S) ? 1u : 0u;          // x-half 1 meets the footprint
-                            uint4 desc;                                                   // address may wrap; valid taps do not
-                            desc.x = tab_addr + (uint32_t)(sub * slice_bytes + ((dy0 + kPad) * sp.pitch + dx0) * 8);
-                            desc.y = __float_as_uint(v.x);
-                            desc.z = __float_as_uint(v.y);
-                            desc.w = 0u;
-                            stage[lane] = desc;
-                            packed = (uint32_t)jl | ((uint32_t)(jh - 1) << 3) | (left << 6) | (right << 7) |
-                                     ((uint32_t)(dx0 & 0xff) << 8);
-                        }
-                    }
-                    unsigned m = __ballot_sync(0xffffffffu, hit);
-                    if (m == 0u) continue;
-                    any = true;
-                    __syncwarp();
-                    while (m) {                                    // m, src, ctrl are warp-uniform by construction
-                        const int src = __ffs(m) - 1;
-                        m &= m - 1;
-                        const uint32_t ctrl = __reduce_or_sync(0xffffffffu, lane == src ? packed : 0u);
-                        const uint4 d = stage[src];                // broadcast LDS.128
-                        const int jl = (int)(ctrl & 7u), jh = (int)((ctrl >> 3) & 7u) + 1;
-                        const int c0 = (int)(int8_t)((ctrl >> 8) & 0xffu) + lx;           // this lane's tap column, x-half 0
-                        const float vr = __uint_as_float(d.y), vi = __uint_as_float(d.z);
-                        const float2 vrr = make_float2(vr, vr), vii = make_float2(vi, vi);
-                        // lanes outside the footprint columns read a zero tap (first pad element) with step 0
-                        const bool v0 = (unsigned)c0 < (unsigned)S, v1 = (unsigned)(c0 + kLaneW) < (unsigned)S;
-                        const uint32_t addr0 = v0 ? d.x + lane_off : tab_addr, step0 = v0 ? (uint32_t)step_bytes : 0u;
-                        const uint32_t addr1 = v1 ? d.x + lane_off + kLaneW * 8 : tab_addr, step1 = v1 ? (uint32_t)step_bytes : 0u;
-                        const uint32_t halves = ctrl & 0xc0u;
-                        if (halves == 0xc0u) {
-                            IMAGER_CHAIN(IMAGER_SLOT_BOTH)
-                        } else if (halves == 0x40u) {
-                            IMAGER_CHAIN(IMAGER_SLOT_LEFT)
-                        } else {
-                            IMAGER_CHAIN(IMAGER_SLOT_RIGHT)
-                        }
-                    }
-                    __syncwarp();
-                }
+            uint32_t touched = 0u;
+            // software pipeline over batches of 32 hits: records and values of the next batch are in flight
+            uint2 rec = make_uint2(0u, 0u);
+            float2 val = make_float2(0.f, 0.f);
+            if (lane < it.hit_count) {
+                rec = a.hit_rec[it.hit_begin + lane];
+                val = sval[(int64_t)rec.x * NC + c_corr];
             }
-            if (any) {
+            for (int b0 = 0; b0 < it.hit_count; b0 += 32) {
+                const int n = min(32, it.hit_count - b0);
+                const uint32_t my_ctrl = lane < n ? rec.y >> 24 : 0x40u;
+                const uint32_t my_variant = ctrl_variant(my_ctrl);
+                stage[lane] = make_uint4(tab_addr + (uint32_t)(((int)(rec.y & 0xffffffu) - (int)kTapBias) * 8) + 0u,
+                                         __float_as_uint(val.x), __float_as_uint(val.y), rec.x);
+                if (lane < n) touched |= ctrl_slot_mask(my_ctrl);
+                if (b0 + 32 + lane < it.hit_count) {
+                    rec = a.hit_rec[it.hit_begin + b0 + 32 + lane];
+                    val = sval[(int64_t)rec.x * NC + c_corr];
+                }
+                __syncwarp();
+                for (int h = 0; h < n;) {                                   // runs of equal variant (the planner sorted them)
+                    const uint32_t variant = __reduce_or_sync(0xffffffffu, lane == h ? my_variant : 0u);   // warp-uniform
+                    const int cnt = __popc(__ballot_sync(0xffffffffu, lane >= h && lane < n && my_variant == variant));
+                    const uint32_t desc_addr = stage_addr + h * 16;
+#define IMAGER_BODY_ARGS (A0, B0, A1, B1, desc_addr, cnt, lane_off, step)
+                    IMAGER_DISPATCH(grid_run, variant)
+#undef IMAGER_BODY_ARGS
+                    h += cnt;
+                }
+                __syncwarp();
+            }
+            touched = __reduce_or_sync(0xffffffffu, touched);
+            const int sy = it.strip / g.strips_per_row, sx = it.strip - sy * g.strips_per_row;
+            float2* gp = gplane + (int64_t)(sy * kStripH + ly) * g.N + sx * kStripW + lx;
 #pragma unroll
-                for (int j = 0; j < kNY; ++j) {
-                    const int64_t cell = (int64_t)(Yw + ly + kLaneH * j) * g.N + Xw + lx;
-                    float re = A0[j].x - B0[j].y, im = A0[j].y + B0[j].x;
-                    if (re != 0.f || im != 0.f) atomicAdd(&grid[cell], make_float2(re, im));
-                    re = A1[j].x - B1[j].y;
-                    im = A1[j].y + B1[j].x;
-                    if (re != 0.f || im != 0.f) atomicAdd(&grid[cell + kLaneW], make_float2(re, im));
+            for (int j = 0; j < kNY; ++j) {
+                if (touched & (1u << j)) {
+                    const float re = A0[j].x - B0[j].y, im = A0[j].y + B0[j].x;
+                    if (re != 0.f || im != 0.f) atomicAdd(gp + (int64_t)(kLaneH * j) * g.N, make_float2(re, im));
+                }
+                if (touched & (0x100u << j)) {
+                    const float re = A1[j].x - B1[j].y, im = A1[j].y + B1[j].x;
+                    if (re != 0.f || im != 0.f) atomicAdd(gp + (int64_t)(kLaneH * j) * g.N + kLaneW, make_float2(re, im));
                 }
             }
         }
@@ -345,67 +505,76 @@ __global__ void __launch_bounds__(kTiledThreads, 1) grid_tiled_kernel(const Tile
 
 struct TiledState {
     std::vector<SetPlan> plan;
-    std::vector<int32_t> unit_set;
+    std::vector<int32_t> gu_set;
     SetPlan* d_plan = nullptr;
-    int32_t* d_unit_set = nullptr;
-    int32_t* d_ref_mask = nullptr;        // per set: 1 = no tiled plan (reference kernels handle it)
-    int32_t* d_parts = nullptr;           // [n_units * n_strips + 1] -> scanned into entry starts
+    int32_t* d_gu_set = nullptr;
+    int32_t* d_hits = nullptr;            // [n_cells + 1] -> scanned into hit starts
+    int32_t* d_items = nullptr;           // [n_cells + 1] -> scanned into item starts
     int32_t* d_scan_tmp = nullptr;
-    Entry* d_entries = nullptr;
+    uint2* d_hit_rec = nullptr;
+    Item* d_item_rec = nullptr;
     Block* d_blocks = nullptr;
-    int64_t max_entries = 0, max_blocks = 0;
+    int64_t cap_hits = 0, cap_items = 0, cap_blocks = 0;
+    int32_t* h_totals = nullptr;          // pinned [2]
     uint2* d_sgeo = nullptr;
     float2* d_sval = nullptr;
-    int64_t geo_epoch = -1;
+    int64_t plan_epoch = -1;
     Geometry g;
     int smem_bytes = 0;
-    bool any_tiled = false, any_ref = false, usable = true;
 };
 
 bool tiled_supported(const imager_plan* pl) {
     const imager_params& p = pl->p;
-    if (!(p.n_corr == 1 && p.n_pol == 1 && p.grid_size % kStripH == 0 && p.grid_size <= 32768 &&
-          p.kernel_mode != IMAGER_MODE_DELTA))
-        return false;
+    if (p.grid_size % kStripH != 0 || p.grid_size > 32768) return false;
+    // every slice (with its padding) must fit in shared memory, and the planner enumerates (gu, strip) pairs
     const int64_t n_strips = (int64_t)(p.grid_size / kStripW) * (p.grid_size / kStripH);
-    return (int64_t)pl->n_sets * p.oversample * p.oversample * n_strips <= kMaxPlanCells;   // conservative (all groups)
+    int64_t n_gu = 0;
+    for (int k = 0; k < pl->n_sets; ++k) {
+        const int S = pl->set_support[k];
+        const int pitch = ((S + 2 * kPadX + 7) / 16) * 16 + 8;
+        const int64_t slice_bytes = (int64_t)(S + 2 * kPadY) * pitch * 8;
+        if (slice_bytes > kTableBudget) return false;
+        int gs = p.oversample * p.oversample;
+        while (gs > 1 && gs * slice_bytes > kTableBudget) gs >>= 1;
+        if ((p.oversample * p.oversample) % gs) return false;
+        n_gu += (p.oversample * p.oversample) / gs;
+    }
+    return n_gu * n_strips <= kMaxPlanCells;
 }
 
 static TiledState* state_of(imager_plan* pl) {
     if (pl->tiled) return static_cast<TiledState*>(pl->tiled);
     TiledState* st = new TiledState();
     const imager_params& p = pl->p;
-    const int O = p.oversample;
+    const int OO = p.oversample * p.oversample;
     st->plan.resize(pl->n_sets);
-    int units = 0;
+    int n_gu = 0;
     for (int k = 0; k < pl->n_sets; ++k) {
         const int S = pl->set_support[k];
-        SetPlan sp;
-        sp.pitch = ((S + 7) / 16) * 16 + 8;                 // smallest value >= S that is 8 mod 16
-        const int64_t slice_bytes = (int64_t)(S + 2 * kPad) * sp.pitch * 8;
-        sp.group_slices = 0;
-        for (int gsl : {O * O, O, 1})
-            if (gsl * slice_bytes <= kMaxSmem - 1024 - kStageBytes) { sp.group_slices = gsl; break; }
-        sp.n_groups = sp.group_slices ? (O * O) / sp.group_slices : 0;
-        sp.unit_base = units;
-        units += sp.n_groups;
-        for (int q = 0; q < sp.n_groups; ++q) st->unit_set.push_back(k);
-        if (sp.group_slices) {
-            st->any_tiled = true;
-            st->smem_bytes = std::max<int>(st->smem_bytes, (int)(sp.group_slices * slice_bytes) + kStageBytes);
-        } else {
-            st->any_ref = true;
-        }
+        SetPlan sp = {};
+        sp.pitch = ((S + 2 * kPadX + 7) / 16) * 16 + 8;      // smallest value >= S + 14 that is 8 mod 16
+        sp.rows = S + 2 * kPadY;
+        const int64_t slice_bytes = (int64_t)sp.rows * sp.pitch * 8;
+        int gs = OO;
+        while (gs > 1 && gs * slice_bytes > kTableBudget) gs >>= 1;
+        sp.group_slices = gs;
+        sp.n_groups = OO / gs;
+        sp.gu_base = n_gu;
+        n_gu += sp.n_groups;
+        for (int q = 0; q < sp.n_groups; ++q) st->gu_set.push_back(k);
+        st->smem_bytes = std::max<int>(st->smem_bytes, (int)(gs * slice_bytes) + kStageBytes);
         st->plan[k] = sp;
     }
     Geometry& g = st->g;
     g.N = p.grid_size;
-    g.O = O;
+    g.O = p.oversample;
     g.nt = pl->nt;
     g.strips_per_row = p.grid_size / kStripW;
     g.n_strips = g.strips_per_row * (p.grid_size / kStripH);
     g.n_sets = pl->n_sets;
-    g.n_units = units;
+    g.n_gu = n_gu;
+    g.n_pol = p.n_pol;
+    g.n_corr = p.n_corr;
     pl->tiled = st;
     return st;
 }
@@ -414,61 +583,109 @@ void tiled_release(imager_plan* pl) {
     if (!pl->tiled) return;
     TiledState* st = static_cast<TiledState*>(pl->tiled);
     cudaFree(st->d_plan);
-    cudaFree(st->d_unit_set);
-    cudaFree(st->d_ref_mask);
-    cudaFree(st->d_parts);
+    cudaFree(st->d_gu_set);
+    cudaFree(st->d_hits);
+    cudaFree(st->d_items);
     cudaFree(st->d_scan_tmp);
-    cudaFree(st->d_entries);
+    cudaFree(st->d_hit_rec);
+    cudaFree(st->d_item_rec);
     cudaFree(st->d_blocks);
     cudaFree(st->d_sgeo);
     cudaFree(st->d_sval);
+    if (st->h_totals) cudaFreeHost(st->h_totals);
     delete st;
     pl->tiled = nullptr;
 }
 
+template <typename T>
+static int grow(T** ptr, int64_t* cap, int64_t need) {
+    if (need <= *cap) return 0;
+    if (*ptr) IMAGER_CUDA(cudaFree(*ptr));
+    *ptr = nullptr;
+    *cap = 0;
+    const int64_t n = need + need / 8 + 1024;
+    IMAGER_CUDA(cudaMalloc(ptr, n * sizeof(T)));
+    *cap = n;
+    return 0;
+}
+
+// (Re)build the hit lists, items and blocks for the current index.  Synchronises the stream once (the sizes of the
+// lists are read back to size their storage); cached until the next re-indexing.
 static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
     const int64_t mv = std::max<int64_t>(pl->p.max_nvis, 1);
     const Geometry& g = st->g;
-    const int64_t n_cells = (int64_t)g.n_units * g.n_strips;
+    const int64_t n_cells = (int64_t)g.n_gu * g.n_strips;
     if (!st->d_plan) {
-        std::vector<int32_t> mask(pl->n_sets);
-        for (int k = 0; k < pl->n_sets; ++k) mask[k] = st->plan[k].group_slices == 0;
         IMAGER_CUDA(cudaMalloc(&st->d_plan, pl->n_sets * sizeof(SetPlan)));
-        IMAGER_CUDA(cudaMalloc(&st->d_ref_mask, pl->n_sets * sizeof(int32_t)));
-        IMAGER_CUDA(cudaMalloc(&st->d_unit_set, std::max<size_t>(1, st->unit_set.size()) * sizeof(int32_t)));
+        IMAGER_CUDA(cudaMalloc(&st->d_gu_set, st->gu_set.size() * sizeof(int32_t)));
         IMAGER_CUDA(cudaMemcpyAsync(st->d_plan, st->plan.data(), pl->n_sets * sizeof(SetPlan), cudaMemcpyHostToDevice, stream));
-        IMAGER_CUDA(cudaMemcpyAsync(st->d_ref_mask, mask.data(), pl->n_sets * sizeof(int32_t), cudaMemcpyHostToDevice, stream));
-        IMAGER_CUDA(cudaMemcpyAsync(st->d_unit_set, st->unit_set.data(), st->unit_set.size() * sizeof(int32_t),
+        IMAGER_CUDA(cudaMemcpyAsync(st->d_gu_set, st->gu_set.data(), st->gu_set.size() * sizeof(int32_t),
                                     cudaMemcpyHostToDevice, stream));
-        IMAGER_CUDA(cudaStreamSynchronize(stream));     // one-off: `mask` goes out of scope
-        // every visibility is a candidate of at most ceil((32+S+W)/W) * ceil((32+S+H)/H) strips; bound with S = 255
-        st->max_entries = n_cells + 2 + (mv * 20 * 11) / kChunk;
-        st->max_blocks = g.n_units + st->max_entries / kBlockEntries + 2;
         int64_t tmp_len = 16;
         for (int64_t n = n_cells + 1; n > 1; n = (n + 1023) / 1024) tmp_len += (n + 1023) / 1024 + 1;
-        IMAGER_CUDA(cudaMalloc(&st->d_parts, (n_cells + 1) * sizeof(int32_t)));
+        IMAGER_CUDA(cudaMalloc(&st->d_hits, (n_cells + 1) * sizeof(int32_t)));
+        IMAGER_CUDA(cudaMalloc(&st->d_items, (n_cells + 1) * sizeof(int32_t)));
         IMAGER_CUDA(cudaMalloc(&st->d_scan_tmp, tmp_len * sizeof(int32_t)));
-        IMAGER_CUDA(cudaMalloc(&st->d_entries, st->max_entries * sizeof(Entry)));
-        IMAGER_CUDA(cudaMalloc(&st->d_blocks, st->max_blocks * sizeof(Block)));
         IMAGER_CUDA(cudaMalloc(&st->d_sgeo, mv * sizeof(uint2)));
         IMAGER_CUDA(cudaMalloc(&st->d_sval, mv * pl->p.n_corr * sizeof(float2)));
-        IMAGER_CUDA(cudaFuncSetAttribute(grid_tiled_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
+        IMAGER_CUDA(cudaMallocHost(&st->h_totals, 2 * sizeof(int32_t)));
+        IMAGER_CUDA(cudaFuncSetAttribute(grid_tiled_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
+        IMAGER_CUDA(cudaFuncSetAttribute(grid_tiled_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
     }
-    if (st->geo_epoch != pl->index_epoch) {
-        sorted_geo_kernel<<<4 * kNumSMs, 256, 0, stream>>>(pl->d_counters, pl->d_perm[pl->sorted_buf], pl->d_rec,
-                                                           pl->p.oversample, st->d_sgeo);
-        const unsigned nb = (unsigned)((n_cells + 1 + 255) / 256);
-        plan_count_kernel<<<nb, 256, 0, stream>>>(g, st->d_plan, st->d_unit_set, pl->d_set_support, pl->d_bucket_offset,
-                                                  st->d_parts);
-        pl->last_launches += 2;
-        int rc = exclusive_scan_i32(pl, st->d_parts, n_cells + 1, st->d_scan_tmp, stream);
-        if (rc) return rc;
-        plan_fill_kernel<<<nb, 256, 0, stream>>>(g, st->d_parts, st->d_entries);
-        plan_blocks_kernel<<<1, 1024, 0, stream>>>(g, st->d_plan, st->d_unit_set, st->d_parts, st->d_blocks, pl->d_counters + 9);
-        pl->last_launches += 2;
-        st->geo_epoch = pl->index_epoch;
+    if (st->plan_epoch == pl->index_epoch) return 0;
+    sorted_geo_kernel<<<4 * kNumSMs, 256, 0, stream>>>(pl->d_counters, pl->d_perm[pl->sorted_buf], pl->d_rec,
+                                                       pl->p.oversample, st->d_sgeo);
+    PlanArgs pa;
+    pa.g = g;
+    pa.set_plan = st->d_plan;
+    pa.gu_set = st->d_gu_set;
+    pa.set_support = pl->d_set_support;
+    pa.bucket_offset = pl->d_bucket_offset;
+    pa.sgeo = st->d_sgeo;
+    const unsigned nb = (unsigned)((n_cells + 1 + 7) / 8);               // 8 warps per thread block
+    plan_hits_kernel<0><<<nb, 256, 0, stream>>>(pa, st->d_hits, st->d_items, nullptr, nullptr);
+    pl->last_launches += 2;
+    int rc = exclusive_scan_i32(pl, st->d_hits, n_cells + 1, st->d_scan_tmp, stream);
+    if (rc) return rc;
+    rc = exclusive_scan_i32(pl, st->d_items, n_cells + 1, st->d_scan_tmp, stream);
+    if (rc) return rc;
+    IMAGER_CUDA(cudaMemcpyAsync(&st->h_totals[0], st->d_hits + n_cells, sizeof(int32_t), cudaMemcpyDeviceToHost, stream));
+    IMAGER_CUDA(cudaMemcpyAsync(&st->h_totals[1], st->d_items + n_cells, sizeof(int32_t), cudaMemcpyDeviceToHost, stream));
+    IMAGER_CUDA(cudaStreamSynchronize(stream));
+    const int64_t n_hits = st->h_totals[0], n_items = st->h_totals[1];
+    if (n_hits < 0 || n_items < 0) {
+        set_error("hit lists exceed 2^31 entries");
+        return IMAGER_ERR_UNSUPPORTED;
     }
+    const int n_sc = g.n_pol * g.n_corr;
+    const int64_t max_blocks = ((int64_t)g.n_gu + n_hits / kBlockHits + 1) * n_sc;
+    rc = grow(&st->d_hit_rec, &st->cap_hits, n_hits + 1);
+    if (rc) return rc;
+    rc = grow(&st->d_item_rec, &st->cap_items, n_items + 1);
+    if (rc) return rc;
+    rc = grow(&st->d_blocks, &st->cap_blocks, max_blocks + 1);
+    if (rc) return rc;
+    plan_hits_kernel<1><<<nb, 256, 0, stream>>>(pa, st->d_hits, st->d_items, st->d_hit_rec, st->d_item_rec);
+    plan_blocks_kernel<<<1, 1024, 0, stream>>>(g, st->d_hits, st->d_items, st->d_item_rec, st->d_blocks, pl->d_counters + 9,
+                                               (int)std::min<int64_t>(st->cap_blocks, 0x7fffffff));
+    pl->last_launches += 2;
+    IMAGER_CUDA(cudaGetLastError());
+    st->plan_epoch = pl->index_epoch;
     return 0;
+}
+
+static void fill_args(imager_plan* pl, TiledState* st, TiledArgs& a, const float2* tab) {
+    a.g = st->g;
+    a.hit_rec = st->d_hit_rec;
+    a.items = st->d_item_rec;
+    a.blocks = st->d_blocks;
+    a.n_blocks = pl->d_counters + 9;
+    a.queue = pl->d_counters + 8;
+    a.tab = tab;
+    a.set_offset = pl->d_set_offset;
+    a.set_support = pl->d_set_support;
+    a.set_plan = st->d_plan;
+    a.gu_set = st->d_gu_set;
 }
 
 int launch_grid_tiled(imager_plan* pl, int64_t nvis, const float2* vis, const float* weights, float2* grid,
@@ -477,27 +694,18 @@ int launch_grid_tiled(imager_plan* pl, int64_t nvis, const float2* vis, const fl
     TiledState* st = state_of(pl);
     int rc = prepare(pl, st, stream);
     if (rc) return rc;
-    if (st->any_ref) {
-        rc = launch_grid_reference(pl, nvis, vis, weights, grid, st->d_ref_mask, stream);   // sets without a tiled plan
-        if (rc) return rc;
-    }
-    if (!st->any_tiled) return 0;
-    gather_values_kernel<1><<<4 * kNumSMs, 256, 0, stream>>>(pl->d_counters, pl->d_perm[pl->sorted_buf], vis, weights, st->d_sval);
+    const unsigned gb = 4 * kNumSMs;
+    if (pl->p.n_corr == 1)
+        gather_values_kernel<1><<<gb, 256, 0, stream>>>(pl->d_counters, pl->d_perm[pl->sorted_buf], vis, weights, st->d_sval);
+    else
+        gather_values_kernel<4><<<gb, 256, 0, stream>>>(pl->d_counters, pl->d_perm[pl->sorted_buf], vis, weights, st->d_sval);
     IMAGER_CUDA(cudaMemsetAsync(pl->d_counters + 8, 0, sizeof(int32_t), stream));
     TiledArgs a;
-    a.g = st->g;
-    a.bucket_offset = pl->d_bucket_offset;
-    a.sgeo = st->d_sgeo;
-    a.sval = st->d_sval;
-    a.tab = pl->d_tab_grid;
-    a.set_offset = pl->d_set_offset;
-    a.set_support = pl->d_set_support;
-    a.set_plan = st->d_plan;
-    a.entries = st->d_entries;
-    a.blocks = st->d_blocks;
-    a.n_blocks = pl->d_counters + 9;
-    a.queue = pl->d_counters + 8;
-    grid_tiled_kernel<<<kNumSMs, kTiledThreads, st->smem_bytes, stream>>>(a, grid);
+    fill_args(pl, st, a, pl->d_tab_grid);
+    if (pl->p.n_corr == 1)
+        grid_tiled_kernel<1><<<kNumSMs, kTiledThreads, st->smem_bytes, stream>>>(a, st->d_sval, grid);
+    else
+        grid_tiled_kernel<4><<<kNumSMs, kTiledThreads, st->smem_bytes, stream>>>(a, st->d_sval, grid);
     pl->last_launches += 2;
     IMAGER_CUDA(cudaGetLastError());
     return 0;
