@@ -333,17 +333,25 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
     return d;
 }
 
+__device__ __forceinline__ uint32_t lds32(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+
 template <int H, int JL, int JH>
 __device__ __forceinline__ void grid_run(float2 (&A0)[kNY], float2 (&B0)[kNY], float2 (&A1)[kNY], float2 (&B1)[kNY],
-                                         uint32_t desc_addr, int cnt, const uint32_t lane_off, const uint32_t step) {
-    uint4 d = lds128(desc_addr);
+                                         uint32_t desc_addr, int cnt, const uint32_t lane_off, const uint32_t (&step)[kNY]) {
+    // descriptor = {value.x, value.y, tap address, sorted index}; only the address of the NEXT hit is prefetched (one
+    // loop-carried register); the value is loaded with the taps and is not needed before the first FFMA2
+    uint32_t a_cur = lds32(desc_addr + 8);
 #pragma unroll 1
-    for (int i = 0; i < cnt; ++i) {
+    do {                                                     // cnt >= 1
+        const float2 v = lds64(desc_addr);
         desc_addr += 16;
-        const uint4 dn = lds128(desc_addr);                  // next descriptor (one past the run at its end: unused)
-        const uint32_t addr = d.x + lane_off;
-        const float vr = __uint_as_float(d.y), vi = __uint_as_float(d.z);
-        const float2 vrr = make_float2(vr, vr), vii = make_float2(vi, vi);
+        const uint32_t a_next = lds32(desc_addr + 8);        // one past the run at its end: unused
+        const uint32_t addr = a_cur + lane_off;
+        const float2 vrr = make_float2(v.x, v.x), vii = make_float2(v.y, v.y);
         // at most 8 tap loads in flight: chunks of 4 slots (both halves) or 8 slots (one half)
         constexpr int kChunk = (H == 3) ? 4 : 8;
 #pragma unroll
@@ -351,8 +359,8 @@ __device__ __forceinline__ void grid_run(float2 (&A0)[kNY], float2 (&B0)[kNY], f
             float2 t0[kChunk], t1[kChunk];
 #pragma unroll
             for (int j = j0; j < j0 + kChunk && j < JH; ++j) {
-                if (H & 1) t0[j - j0] = lds64(addr + j * step);
-                if (H & 2) t1[j - j0] = lds64(addr + j * step + kLaneW * 8);
+                if (H & 1) t0[j - j0] = lds64(addr + step[j]);
+                if (H & 2) t1[j - j0] = lds64(addr + step[j] + kLaneW * 8);
             }
 #pragma unroll
             for (int j = j0; j < j0 + kChunk && j < JH; ++j) {
@@ -366,8 +374,8 @@ __device__ __forceinline__ void grid_run(float2 (&A0)[kNY], float2 (&B0)[kNY], f
                 }
             }
         }
-        d = dn;
-    }
+        a_cur = a_next;
+    } while (--cnt > 0);
 }
 
 #define IMAGER_CASE(FN, H, JL, JH1) \
@@ -441,7 +449,11 @@ grid_tiled_kernel(const TiledArgs a, const float2* __restrict__ sval, float2* __
         }
         const int s_pol = blk.sc / g.n_corr, c_corr = blk.sc - s_pol * g.n_corr;
         float2* gplane = grid + (int64_t)s_pol * g.N * g.N;
-        const uint32_t step = (uint32_t)(kLaneH * sp.pitch * 8);              // one slot down
+        // byte offsets of the 8 slots; each REDUX yields a uniform register, so that a tap load is LDS [R + UR] with
+        // no per-slot address arithmetic
+        uint32_t step[kNY];
+#pragma unroll
+        for (int j = 0; j < kNY; ++j) step[j] = __reduce_or_sync(0xffffffffu, (uint32_t)(j * kLaneH * sp.pitch * 8));
         const uint32_t lane_off = (uint32_t)((ly * sp.pitch + lx) * 8);
         for (;;) {
             int ii = 0;
@@ -453,24 +465,23 @@ grid_tiled_kernel(const TiledArgs a, const float2* __restrict__ sval, float2* __
 #pragma unroll
             for (int j = 0; j < kNY; ++j) A0[j] = B0[j] = A1[j] = B1[j] = make_float2(0.f, 0.f);
             uint32_t touched = 0u;
-            // software pipeline over batches of 32 hits: records and values of the next batch are in flight
-            uint2 rec = make_uint2(0u, 0u);
+            // software pipeline over batches of 32 hits: the records of batch b + 2 and the values of batch b + 1 are
+            // in flight while batch b is replayed
+            uint2 rec = make_uint2(0u, 0u), rec1 = make_uint2(0u, 0u);
             float2 val = make_float2(0.f, 0.f);
-            if (lane < it.hit_count) {
-                rec = a.hit_rec[it.hit_begin + lane];
-                val = sval[(int64_t)rec.x * NC + c_corr];
-            }
+            if (lane < it.hit_count) rec = a.hit_rec[it.hit_begin + lane];
+            if (lane + 32 < it.hit_count) rec1 = a.hit_rec[it.hit_begin + 32 + lane];
+            if (lane < it.hit_count) val = sval[(int64_t)rec.x * NC + c_corr];
             for (int b0 = 0; b0 < it.hit_count; b0 += 32) {
                 const int n = min(32, it.hit_count - b0);
                 const uint32_t my_ctrl = lane < n ? rec.y >> 24 : 0x40u;
                 const uint32_t my_variant = ctrl_variant(my_ctrl);
-                stage[lane] = make_uint4(tab_addr + (uint32_t)(((int)(rec.y & 0xffffffu) - (int)kTapBias) * 8) + 0u,
-                                         __float_as_uint(val.x), __float_as_uint(val.y), rec.x);
+                stage[lane] = make_uint4(__float_as_uint(val.x), __float_as_uint(val.y),
+                                         tab_addr + (uint32_t)(((int)(rec.y & 0xffffffu) - (int)kTapBias) * 8), rec.x);
                 if (lane < n) touched |= ctrl_slot_mask(my_ctrl);
-                if (b0 + 32 + lane < it.hit_count) {
-                    rec = a.hit_rec[it.hit_begin + b0 + 32 + lane];
-                    val = sval[(int64_t)rec.x * NC + c_corr];
-                }
+                rec = rec1;
+                if (b0 + 32 + lane < it.hit_count) val = sval[(int64_t)rec.x * NC + c_corr];
+                if (b0 + 64 + lane < it.hit_count) rec1 = a.hit_rec[it.hit_begin + b0 + 64 + lane];
                 __syncwarp();
                 for (int h = 0; h < n;) {                                   // runs of equal variant (the planner sorted them)
                     const uint32_t variant = __reduce_or_sync(0xffffffffu, lane == h ? my_variant : 0u);   // warp-uniform
