@@ -34,7 +34,7 @@ constexpr int kItemHits = 128;                        // hits per work item (one
 constexpr int kBlockHits = 16384;                     // hits per CTA-level block
 constexpr int kStageBytes = kWarps * 32 * 16;         // per-warp hit descriptors
 constexpr int kMaxSmem = 227 * 1024;
-constexpr int kTableBudget = kMaxSmem - kStageBytes - 1024;
+constexpr int kTableBudget = kMaxSmem - kStageBytes - 32 * 1024 - 1024;   // stage + degridding reduction buffer + static
 constexpr int64_t kMaxPlanCells = 48 << 20;           // (geometry unit, strip) pairs the planner may enumerate
 constexpr uint32_t kTapBias = 1u << 20;
 
@@ -512,6 +512,173 @@ grid_tiled_kernel(const TiledArgs a, const float2* __restrict__ sval, float2* __
     }
 }
 
+// ---- degridding ------------------------------------------------------------------------------------------
+// Same hits, same ownership: the warp holds its strip of the grid in registers; a hit's lanes accumulate
+// sum conj(t) g over their cells:  P += t * g.x, Q += t * g.y,  conj(t) g = (P.x + Q.y) + i (Q.x - P.y).
+// The 32 partial sums of a hit go to a per-warp shared buffer red[slot][lane]; every 8 hits the buffer is summed
+// by a transposed read (lane = slot + 8 * quarter sums 8 columns, two shuffles join the quarters) and the result is
+// added to the visibility's sorted-order sum with one red.global.add.v2.f32 per hit.
+constexpr int kRedSlots = 8;
+constexpr int kRedBytes = kWarps * kRedSlots * 32 * 8;      // 32 KB
+
+__device__ __forceinline__ void sts64(uint32_t addr, float2 v) {
+    asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(v.x), "f"(v.y) : "memory");
+}
+
+template <int H, int JL, int JH>
+__device__ __forceinline__ void degrid_run(const float2 (&G0)[kNY], const float2 (&G1)[kNY], uint32_t desc_addr, int cnt,
+                                           uint32_t red_addr, const uint32_t lane_off, const uint32_t (&step)[kNY]) {
+    uint32_t a_cur = lds32(desc_addr);
+#pragma unroll 1
+    do {                                                     // cnt >= 1
+        desc_addr += 8;
+        const uint32_t a_next = lds32(desc_addr);            // one past the run at its end: unused
+        const uint32_t addr = a_cur + lane_off;
+        float2 P0 = make_float2(0.f, 0.f), Q0 = P0, P1 = P0, Q1 = P0;
+        constexpr int kChunk = (H == 3) ? 4 : 8;
+#pragma unroll
+        for (int j0 = JL; j0 < JH; j0 += kChunk) {
+            float2 t0[kChunk], t1[kChunk];
+#pragma unroll
+            for (int j = j0; j < j0 + kChunk && j < JH; ++j) {
+                if (H & 1) t0[j - j0] = lds64(addr + step[j]);
+                if (H & 2) t1[j - j0] = lds64(addr + step[j] + kLaneW * 8);
+            }
+#pragma unroll
+            for (int j = j0; j < j0 + kChunk && j < JH; ++j) {
+                if (H & 1) {
+                    ffma2(P0, t0[j - j0], make_float2(G0[j].x, G0[j].x));
+                    ffma2(Q0, t0[j - j0], make_float2(G0[j].y, G0[j].y));
+                }
+                if (H & 2) {
+                    ffma2(P1, t1[j - j0], make_float2(G1[j].x, G1[j].x));
+                    ffma2(Q1, t1[j - j0], make_float2(G1[j].y, G1[j].y));
+                }
+            }
+        }
+        float re, im;
+        if (H == 3) {
+            re = (P0.x + Q0.y) + (P1.x + Q1.y);
+            im = (Q0.x - P0.y) + (Q1.x - P1.y);
+        } else if (H == 1) {
+            re = P0.x + Q0.y;
+            im = Q0.x - P0.y;
+        } else {
+            re = P1.x + Q1.y;
+            im = Q1.x - P1.y;
+        }
+        sts64(red_addr, make_float2(re, im));
+        red_addr += 32 * 8;
+        a_cur = a_next;
+    } while (--cnt > 0);
+}
+
+template <int NC>
+__global__ void __launch_bounds__(kTiledThreads, 1)
+degrid_tiled_kernel(const TiledArgs a, const float2* __restrict__ grid, float2* __restrict__ ssum) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5;
+    uint2* stage = reinterpret_cast<uint2*>(smem_raw) + warp * 32;                       // {tap address, sorted index}
+    float2* red = reinterpret_cast<float2*>(smem_raw + kStageBytes) + warp * kRedSlots * 32;
+    float2* tab_s = reinterpret_cast<float2*>(smem_raw + kStageBytes + kRedBytes);
+    const uint32_t tab_addr = (uint32_t)__cvta_generic_to_shared(tab_s);
+    const uint32_t stage_addr = (uint32_t)__cvta_generic_to_shared(stage);
+    const uint32_t red_base = (uint32_t)__cvta_generic_to_shared(red);
+    __shared__ int s_block, s_next;
+    const int lane = threadIdx.x & 31, lx = lane & (kLaneW - 1), ly = lane >> 3;
+    const Geometry g = a.g;
+    const int n_blocks = *a.n_blocks;
+    int cur_gu = -1, cur_sc = -1;
+    for (;;) {
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            s_block = atomicAdd(a.queue, 1);
+            s_next = 0;
+        }
+        __syncthreads();
+        if (s_block >= n_blocks) break;
+        const Block blk = a.blocks[s_block];
+        const int kset = a.gu_set[blk.gu];
+        const SetPlan sp = a.set_plan[kset];
+        const int S = a.set_support[kset];
+        if (blk.gu != cur_gu || blk.sc != cur_sc) {
+            load_table_group(a, kset, blk.gu - sp.gu_base, blk.sc, sp, S, tab_s);
+            cur_gu = blk.gu;
+            cur_sc = blk.sc;
+            __syncthreads();
+        }
+        const int s_pol = blk.sc / g.n_corr, c_corr = blk.sc - s_pol * g.n_corr;
+        const float2* gplane = grid + (int64_t)s_pol * g.N * g.N;
+        uint32_t step[kNY];
+#pragma unroll
+        for (int j = 0; j < kNY; ++j) step[j] = __reduce_or_sync(0xffffffffu, (uint32_t)(j * kLaneH * sp.pitch * 8));
+        const uint32_t lane_off = (uint32_t)((ly * sp.pitch + lx) * 8);
+        for (;;) {
+            int ii = 0;
+            if (lane == 0) ii = atomicAdd(&s_next, 1);
+            ii = __shfl_sync(0xffffffffu, ii, 0);
+            if (ii >= blk.item_count) break;
+            const Item it = a.items[blk.item_begin + ii];
+            const int sy = it.strip / g.strips_per_row, sx = it.strip - sy * g.strips_per_row;
+            const float2* gp = gplane + (int64_t)(sy * kStripH + ly) * g.N + sx * kStripW + lx;
+            float2 G0[kNY], G1[kNY];
+#pragma unroll
+            for (int j = 0; j < kNY; ++j) {
+                G0[j] = __ldg(gp + (int64_t)(kLaneH * j) * g.N);
+                G1[j] = __ldg(gp + (int64_t)(kLaneH * j) * g.N + kLaneW);
+            }
+            uint2 rec = make_uint2(0u, 0u), rec1 = make_uint2(0u, 0u);
+            if (lane < it.hit_count) rec = a.hit_rec[it.hit_begin + lane];
+            if (lane + 32 < it.hit_count) rec1 = a.hit_rec[it.hit_begin + 32 + lane];
+            for (int b0 = 0; b0 < it.hit_count; b0 += 32) {
+                const int n = min(32, it.hit_count - b0);
+                const uint32_t my_ctrl = lane < n ? rec.y >> 24 : 0x40u;
+                const uint32_t my_variant = ctrl_variant(my_ctrl);
+                stage[lane] = make_uint2(tab_addr + (uint32_t)(((int)(rec.y & 0xffffffu) - (int)kTapBias) * 8), rec.x);
+                rec = rec1;
+                if (b0 + 64 + lane < it.hit_count) rec1 = a.hit_rec[it.hit_begin + b0 + 64 + lane];
+                __syncwarp();
+                for (int h = 0; h < n;) {
+                    const uint32_t variant = __reduce_or_sync(0xffffffffu, lane == h ? my_variant : 0u);   // warp-uniform
+                    int cnt = __popc(__ballot_sync(0xffffffffu, lane >= h && lane < n && my_variant == variant));
+                    cnt = min(cnt, kRedSlots - (h & (kRedSlots - 1)));          // runs do not cross a reduction batch
+                    const uint32_t desc_addr = stage_addr + h * 8;
+                    const uint32_t red_addr = red_base + (uint32_t)(((h & (kRedSlots - 1)) * 32 + lane) * 8);
+#define IMAGER_BODY_ARGS (G0, G1, desc_addr, cnt, red_addr, lane_off, step)
+                    IMAGER_DISPATCH(degrid_run, variant)
+#undef IMAGER_BODY_ARGS
+                    h += cnt;
+                    if ((h & (kRedSlots - 1)) == 0 || h == n) {
+                        // transposed reduction of hits [h0, h): lane = slot + 8 * quarter sums columns 8 q .. 8 q + 7
+                        const int h0 = (h - 1) & ~(kRedSlots - 1);
+                        __syncwarp();
+                        const int slot = lane & (kRedSlots - 1), q = lane >> 3;
+                        float2 acc = make_float2(0.f, 0.f);
+                        if (h0 + slot < h) {
+#pragma unroll
+                            for (int k = 0; k < 8; ++k) {
+                                const float2 v = lds64(red_base + (uint32_t)((slot * 32 + 8 * q + ((k + slot) & 7)) * 8));
+                                acc.x += v.x;
+                                acc.y += v.y;
+                            }
+                        }
+                        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 8);
+                        acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 8);
+                        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 16);
+                        acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 16);
+                        if (lane < kRedSlots && h0 + lane < h) {
+                            const uint32_t idx = stage[h0 + lane].y;
+                            atomicAdd(&ssum[(int64_t)idx * NC + c_corr], acc);
+                        }
+                        __syncwarp();
+                    }
+                }
+                __syncwarp();
+            }
+        }
+    }
+}
+
 // ---- host side -------------------------------------------------------------------------------------------
 
 struct TiledState {
@@ -642,6 +809,8 @@ static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
         IMAGER_CUDA(cudaMallocHost(&st->h_totals, 2 * sizeof(int32_t)));
         IMAGER_CUDA(cudaFuncSetAttribute(grid_tiled_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
         IMAGER_CUDA(cudaFuncSetAttribute(grid_tiled_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
+        IMAGER_CUDA(cudaFuncSetAttribute(degrid_tiled_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
+        IMAGER_CUDA(cudaFuncSetAttribute(degrid_tiled_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
     }
     if (st->plan_epoch == pl->index_epoch) return 0;
     sorted_geo_kernel<<<4 * kNumSMs, 256, 0, stream>>>(pl->d_counters, pl->d_perm[pl->sorted_buf], pl->d_rec,
@@ -723,7 +892,27 @@ int launch_grid_tiled(imager_plan* pl, int64_t nvis, const float2* vis, const fl
 }
 
 int launch_degrid_tiled(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, cudaStream_t stream) {
-    return launch_degrid_reference(pl, nvis, grid, vis_out, nullptr, stream);
+    if (nvis == 0) return 0;
+    TiledState* st = state_of(pl);
+    int rc = prepare(pl, st, stream);
+    if (rc) return rc;
+    const int nc = pl->p.n_corr;
+    IMAGER_CUDA(cudaMemsetAsync(st->d_sval, 0, (size_t)nvis * nc * sizeof(float2), stream));
+    IMAGER_CUDA(cudaMemsetAsync(pl->d_counters + 8, 0, sizeof(int32_t), stream));
+    TiledArgs a;
+    fill_args(pl, st, a, pl->d_tab_degrid);
+    const int smem = st->smem_bytes + kRedBytes;
+    const unsigned gb = 4 * kNumSMs;
+    if (nc == 1) {
+        degrid_tiled_kernel<1><<<kNumSMs, kTiledThreads, smem, stream>>>(a, grid, st->d_sval);
+        scatter_values_kernel<1><<<gb, 256, 0, stream>>>(nvis, pl->d_counters, pl->d_perm[pl->sorted_buf], st->d_sval, vis_out);
+    } else {
+        degrid_tiled_kernel<4><<<kNumSMs, kTiledThreads, smem, stream>>>(a, grid, st->d_sval);
+        scatter_values_kernel<4><<<gb, 256, 0, stream>>>(nvis, pl->d_counters, pl->d_perm[pl->sorted_buf], st->d_sval, vis_out);
+    }
+    pl->last_launches += 2;
+    IMAGER_CUDA(cudaGetLastError());
+    return 0;
 }
 
 }  // namespace imager
