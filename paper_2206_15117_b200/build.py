@@ -48,5 +48,17 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def build_probe() -> str:
+    """The operand-port micro-benchmarks quoted in DESIGN.md / profiles/r1_port_probe.md (a standalone executable)."""
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    exe = os.path.join(HERE, "port_probe")
+    subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
+                           os.path.join(CSRC, "port_probe.cu"), "-o", exe])
+    return exe
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--probe" in sys.argv:
+        print(build_probe())
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
