@@ -53,8 +53,10 @@ enum {
 enum {
     IMAGER_REUSE_INDEX = 1u,        /* uvw / a_index / nvis unchanged since the previous grid or degrid call on this
                                        plan: skip indexing and bucketing (the steady state of a major-cycle loop) */
-    IMAGER_PATH_REFERENCE = 2u      /* use the simple one-warp-per-visibility kernels instead of the tiled ones
+    IMAGER_PATH_REFERENCE = 2u,     /* use the simple one-warp-per-visibility kernels instead of the tiled ones
                                        (same results up to summation order; for tests and A/B timing)             */
+    IMAGER_PATH_SMEM = 4u           /* use the shared-memory-tap tiled kernels instead of the TMEM-tap ones (the
+                                       fallback for shapes whose slices do not fit a TMEM lane; A/B timing)       */
 };
 
 typedef struct imager_plan imager_plan;   /* opaque, owned by the library */
