@@ -55,8 +55,10 @@ enum {
                                        plan: skip indexing and bucketing (the steady state of a major-cycle loop) */
     IMAGER_PATH_REFERENCE = 2u,     /* use the simple one-warp-per-visibility kernels instead of the tiled ones
                                        (same results up to summation order; for tests and A/B timing)             */
-    IMAGER_PATH_SMEM = 4u           /* use the shared-memory-tap tiled kernels instead of the TMEM-tap ones (the
-                                       fallback for shapes whose slices do not fit a TMEM lane; A/B timing)       */
+    IMAGER_PATH_SMEM = 4u,          /* use the shared-memory-tap tiled kernels (the default path; kept so that
+                                       callers can name it explicitly)                                            */
+    IMAGER_PATH_TMEM = 8u           /* gridding with the taps in tensor memory (experimental, slower than the
+                                       default on sparse uv coverage; shapes that do not fit fall back; A/B timing) */
 };
 
 typedef struct imager_plan imager_plan;   /* opaque, owned by the library */

@@ -19,6 +19,7 @@ MODE_DELTA, MODE_PSWF, MODE_WPROJ, MODE_AWPROJ_ADJOINT, MODE_AWPROJ_PAPER, MODE_
 REUSE_INDEX = 1
 PATH_REFERENCE = 2
 PATH_SMEM = 4
+PATH_TMEM = 8
 
 EXPORTS = ("imager_plan_create", "imager_grid", "imager_degrid", "imager_plan_destroy",
            "imager_grid_image_transform", "imager_debug_index", "imager_debug_kernels", "imager_plan_info",

@@ -186,7 +186,7 @@ extern "C" int imager_grid(imager_plan* plan, int64_t nvis, const float* uvw, co
     if (rc) return rc;
     rc = launch_sum_weights(plan, nvis, weights, sum_weights, st);
     if (rc) return rc;
-    if (!(flags & (IMAGER_PATH_REFERENCE | IMAGER_PATH_SMEM)) && tmem_supported(plan))
+    if ((flags & IMAGER_PATH_TMEM) && !(flags & IMAGER_PATH_REFERENCE) && tmem_supported(plan))
         return launch_grid_tmem(plan, nvis, (const float2*)vis, weights, (float2*)grid, st);
     if (!(flags & IMAGER_PATH_REFERENCE) && tiled_supported(plan))
         return launch_grid_tiled(plan, nvis, (const float2*)vis, weights, (float2*)grid, st);
