@@ -30,9 +30,21 @@ constexpr int kNX = 2, kNY = 8;                       // replications: strip = 1
 constexpr int kStripW = kLaneW * kNX, kStripH = kLaneH * kNY;
 constexpr int kPadY = kLaneH - 1, kPadX = kLaneW - 1;
 constexpr int kTiledThreads = 512, kWarps = kTiledThreads / 32;
-constexpr int kItemHits = 128;                        // hits per work item (one flush / strip load each)
-constexpr int kBlockHits = 16384;                     // hits per CTA-level block
-constexpr int kStageBytes = kWarps * 32 * 16;         // per-warp hit descriptors
+#ifndef IMAGER_GRID_THREADS
+#define IMAGER_GRID_THREADS 768
+#endif
+constexpr int kGridThreads = IMAGER_GRID_THREADS;     // gridding kernel: threads per CTA (one CTA per SM)
+#ifndef IMAGER_ITEM_HITS
+#define IMAGER_ITEM_HITS 256
+#endif
+#ifndef IMAGER_BLOCK_HITS
+#define IMAGER_BLOCK_HITS 32768
+#endif
+constexpr int kItemHits = IMAGER_ITEM_HITS;                        // hits per work item (one flush / strip load each)
+constexpr int kBlockHits = IMAGER_BLOCK_HITS;                     // hits per CTA-level block
+constexpr int kStageBytes = kWarps * 32 * 16;         // per-warp hit descriptors (degridding)
+constexpr int kStageSlots = 40;                       // gridding: 32 descriptors + the one read past a batch's end
+constexpr int kGridStageBytes = (kGridThreads / 32) * kStageSlots * 16;
 constexpr int kMaxSmem = 227 * 1024;
 constexpr int kTableBudget = kMaxSmem - kStageBytes - 32 * 1024 - 1024;   // stage + degridding reduction buffer + static
 constexpr int64_t kMaxPlanCells = 48 << 20;           // (geometry unit, strip) pairs the planner may enumerate
@@ -339,19 +351,39 @@ __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
     return v;
 }
 
+typedef unsigned long long u64;
+
+__device__ __forceinline__ u64 pack2(float x, float y) {
+    u64 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(x), "f"(y));
+    return r;
+}
+
+__device__ __forceinline__ float2 unpack2(u64 v) {
+    float2 r;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
+    return r;
+}
+
+__device__ __forceinline__ void ffma2p(u64& d, u64 a, u64 b) { asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(d) : "l"(a), "l"(b)); }
+
+// One complex MAC  acc += t * v  as two FFMA2 on ONE packed accumulator: acc += (t.re, t.im) * (v.re, v.re), then
+// acc += (t.im, t.re) * (-v.im, v.im).  ptxas folds the swapped pair and the sign pattern into operand modifiers
+// (FFMA2 R, -R.F32x2.LO_HI.NP, R.F32, R): no extra instruction, two registers per owned cell.
+__device__ __forceinline__ void cmac_re(u64& acc, float2 t, float vr) { ffma2p(acc, pack2(t.x, t.y), pack2(vr, vr)); }
+__device__ __forceinline__ void cmac_im(u64& acc, float2 t, float vi) { ffma2p(acc, pack2(t.y, t.x), pack2(-vi, vi)); }
+
+// A run: `cnt` consecutive staged hits with the same slot range.  A hit's descriptor {value.x, value.y, tap address, -}
+// is ONE broadcast LDS.128 (one wavefront), loaded a hit ahead; `d` carries the prefetched descriptor across runs.
 template <int H, int JL, int JH>
-__device__ __forceinline__ void grid_run(float2 (&A0)[kNY], float2 (&B0)[kNY], float2 (&A1)[kNY], float2 (&B1)[kNY],
-                                         uint32_t desc_addr, int cnt, const uint32_t lane_off, const uint32_t (&step)[kNY]) {
-    // descriptor = {value.x, value.y, tap address, sorted index}; only the address of the NEXT hit is prefetched (one
-    // loop-carried register); the value is loaded with the taps and is not needed before the first FFMA2
-    uint32_t a_cur = lds32(desc_addr + 8);
+__device__ __forceinline__ void grid_run(u64 (&C0)[kNY], u64 (&C1)[kNY], uint4& d, uint32_t desc_addr, int cnt,
+                                         const uint32_t lane_off, const uint32_t (&step)[kNY]) {
 #pragma unroll 1
     do {                                                     // cnt >= 1
-        const float2 v = lds64(desc_addr);
+        const uint32_t addr = d.z + lane_off;
+        const float vx = __uint_as_float(d.x), vy = __uint_as_float(d.y);
         desc_addr += 16;
-        const uint32_t a_next = lds32(desc_addr + 8);        // one past the run at its end: unused
-        const uint32_t addr = a_cur + lane_off;
-        const float2 vrr = make_float2(v.x, v.x), vii = make_float2(v.y, v.y);
+        d = lds128(desc_addr);                               // the next hit of the batch (one past it at its end: unused)
         // at most 8 tap loads in flight: chunks of 4 slots (both halves) or 8 slots (one half)
         constexpr int kChunk = (H == 3) ? 4 : 8;
 #pragma unroll
@@ -364,17 +396,15 @@ __device__ __forceinline__ void grid_run(float2 (&A0)[kNY], float2 (&B0)[kNY], f
             }
 #pragma unroll
             for (int j = j0; j < j0 + kChunk && j < JH; ++j) {
-                if (H & 1) {
-                    ffma2(A0[j], t0[j - j0], vrr);
-                    ffma2(B0[j], t0[j - j0], vii);
-                }
-                if (H & 2) {
-                    ffma2(A1[j], t1[j - j0], vrr);
-                    ffma2(B1[j], t1[j - j0], vii);
-                }
+                if (H & 1) cmac_re(C0[j], t0[j - j0], vx);
+                if (H & 2) cmac_re(C1[j], t1[j - j0], vx);
+            }
+#pragma unroll
+            for (int j = j0; j < j0 + kChunk && j < JH; ++j) {
+                if (H & 1) cmac_im(C0[j], t0[j - j0], vy);
+                if (H & 2) cmac_im(C1[j], t1[j - j0], vy);
             }
         }
-        a_cur = a_next;
     } while (--cnt > 0);
 }
 
@@ -417,11 +447,11 @@ struct WarpCtx {
 };
 
 template <int NC>
-__global__ void __launch_bounds__(kTiledThreads, 1)
+__global__ void __launch_bounds__(kGridThreads, 1)
 grid_tiled_kernel(const TiledArgs a, const float2* __restrict__ sval, float2* __restrict__ grid) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    uint4* stage = reinterpret_cast<uint4*>(smem_raw) + (threadIdx.x >> 5) * 32;       // this warp's descriptors
-    float2* tab_s = reinterpret_cast<float2*>(smem_raw + kStageBytes);
+    uint4* stage = reinterpret_cast<uint4*>(smem_raw) + (threadIdx.x >> 5) * kStageSlots;  // this warp's descriptors
+    float2* tab_s = reinterpret_cast<float2*>(smem_raw + kGridStageBytes);
     const uint32_t tab_addr = (uint32_t)__cvta_generic_to_shared(tab_s);
     const uint32_t stage_addr = (uint32_t)__cvta_generic_to_shared(stage);
     __shared__ int s_block, s_next;
@@ -461,12 +491,12 @@ grid_tiled_kernel(const TiledArgs a, const float2* __restrict__ sval, float2* __
             ii = __shfl_sync(0xffffffffu, ii, 0);
             if (ii >= blk.item_count) break;
             const Item it = a.items[blk.item_begin + ii];
-            float2 A0[kNY], B0[kNY], A1[kNY], B1[kNY];
+            u64 C0[kNY], C1[kNY];
 #pragma unroll
-            for (int j = 0; j < kNY; ++j) A0[j] = B0[j] = A1[j] = B1[j] = make_float2(0.f, 0.f);
+            for (int j = 0; j < kNY; ++j) C0[j] = C1[j] = 0ull;
             uint32_t touched = 0u;
-            // software pipeline over batches of 32 hits: the records of batch b + 2 and the values of batch b + 1 are
-            // in flight while batch b is replayed
+            // software pipeline over batches of 32 hits (one per lane): the records of batch b + 2 and the values of
+            // batch b + 1 are in flight while batch b is replayed
             uint2 rec = make_uint2(0u, 0u), rec1 = make_uint2(0u, 0u);
             float2 val = make_float2(0.f, 0.f);
             if (lane < it.hit_count) rec = a.hit_rec[it.hit_begin + lane];
@@ -483,11 +513,12 @@ grid_tiled_kernel(const TiledArgs a, const float2* __restrict__ sval, float2* __
                 if (b0 + 32 + lane < it.hit_count) val = sval[(int64_t)rec.x * NC + c_corr];
                 if (b0 + 64 + lane < it.hit_count) rec1 = a.hit_rec[it.hit_begin + b0 + 64 + lane];
                 __syncwarp();
+                uint4 d = lds128(stage_addr);
                 for (int h = 0; h < n;) {                                   // runs of equal variant (the planner sorted them)
                     const uint32_t variant = __reduce_or_sync(0xffffffffu, lane == h ? my_variant : 0u);   // warp-uniform
                     const int cnt = __popc(__ballot_sync(0xffffffffu, lane >= h && lane < n && my_variant == variant));
                     const uint32_t desc_addr = stage_addr + h * 16;
-#define IMAGER_BODY_ARGS (A0, B0, A1, B1, desc_addr, cnt, lane_off, step)
+#define IMAGER_BODY_ARGS (C0, C1, d, desc_addr, cnt, lane_off, step)
                     IMAGER_DISPATCH(grid_run, variant)
 #undef IMAGER_BODY_ARGS
                     h += cnt;
@@ -500,12 +531,12 @@ grid_tiled_kernel(const TiledArgs a, const float2* __restrict__ sval, float2* __
 #pragma unroll
             for (int j = 0; j < kNY; ++j) {
                 if (touched & (1u << j)) {
-                    const float re = A0[j].x - B0[j].y, im = A0[j].y + B0[j].x;
-                    if (re != 0.f || im != 0.f) atomicAdd(gp + (int64_t)(kLaneH * j) * g.N, make_float2(re, im));
+                    const float2 c = unpack2(C0[j]);
+                    if (c.x != 0.f || c.y != 0.f) atomicAdd(gp + (int64_t)(kLaneH * j) * g.N, c);
                 }
                 if (touched & (0x100u << j)) {
-                    const float re = A1[j].x - B1[j].y, im = A1[j].y + B1[j].x;
-                    if (re != 0.f || im != 0.f) atomicAdd(gp + (int64_t)(kLaneH * j) * g.N + kLaneW, make_float2(re, im));
+                    const float2 c = unpack2(C1[j]);
+                    if (c.x != 0.f || c.y != 0.f) atomicAdd(gp + (int64_t)(kLaneH * j) * g.N + kLaneW, c);
                 }
             }
         }
@@ -883,9 +914,9 @@ int launch_grid_tiled(imager_plan* pl, int64_t nvis, const float2* vis, const fl
     TiledArgs a;
     fill_args(pl, st, a, pl->d_tab_grid);
     if (pl->p.n_corr == 1)
-        grid_tiled_kernel<1><<<kNumSMs, kTiledThreads, st->smem_bytes, stream>>>(a, st->d_sval, grid);
+        grid_tiled_kernel<1><<<kNumSMs, kGridThreads, st->smem_bytes - kStageBytes + kGridStageBytes, stream>>>(a, st->d_sval, grid);
     else
-        grid_tiled_kernel<4><<<kNumSMs, kTiledThreads, st->smem_bytes, stream>>>(a, st->d_sval, grid);
+        grid_tiled_kernel<4><<<kNumSMs, kGridThreads, st->smem_bytes - kStageBytes + kGridStageBytes, stream>>>(a, st->d_sval, grid);
     pl->last_launches += 2;
     IMAGER_CUDA(cudaGetLastError());
     return 0;
