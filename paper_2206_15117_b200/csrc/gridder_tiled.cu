@@ -80,13 +80,16 @@ __device__ __forceinline__ float2 lds64(uint32_t addr) {
     return v;
 }
 
-// sorted-order geometry: word0 = gx | gy << 16, word1 = oy_idx * O + ox_idx  (kept visibilities only)
+// sorted-order geometry: word0 = gx | gy << 16, word1 = (oy_idx * O + ox_idx) | kernel set << kSubBits  (kept visibilities)
+constexpr int kSubBits = 14;                          // O <= 128: sub-cell slice index < 2^14
+constexpr uint32_t kSubMask = (1u << kSubBits) - 1u;
 __global__ void sorted_geo_kernel(const int32_t* __restrict__ counters, const int32_t* __restrict__ perm,
                                   const imager_record* __restrict__ rec, int O, uint2* __restrict__ sgeo) {
     const int n_kept = counters[0];
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_kept; i += gridDim.x * blockDim.x) {
         const imager_record r = rec[perm[i]];
-        sgeo[i] = make_uint2((uint32_t)r.gx | ((uint32_t)r.gy << 16), ((r.sub >> 8) & 255u) * O + (r.sub & 255u));
+        sgeo[i] = make_uint2((uint32_t)r.gx | ((uint32_t)r.gy << 16),
+                             (((r.sub >> 8) & 255u) * O + (r.sub & 255u)) | ((uint32_t)r.kset << kSubBits));
     }
 }
 
@@ -167,144 +170,152 @@ __device__ __forceinline__ uint32_t ctrl_variant(uint32_t ctrl) {
     return (uint32_t)IMAGER_VARIANT(h, jl, jh1);
 }
 
-// MODE 0: count hits (hits[cell], items[cell]); MODE 1: write hit records, SORTED BY VARIANT within the cell (stable:
-// candidate order is kept within a variant, so the result is deterministic), and the items.  One warp per (gu, strip).
-template <int MODE>
-__global__ void __launch_bounds__(256) plan_hits_kernel(const PlanArgs a, int32_t* __restrict__ hits, int32_t* __restrict__ items,
-                                                        uint2* __restrict__ hit_rec, Item* __restrict__ item_rec) {
-    __shared__ int32_t s_bin[8][128];
+// Hit counts per (gu, strip), visibility-centric: every kept visibility adds 1 to each strip its footprint meets
+// (about 4 atomics per visibility; sorted order makes neighbouring threads meet the same few counters in L2).
+__global__ void count_hits_kernel(const PlanArgs a, const int32_t* __restrict__ counters, int32_t* __restrict__ hits) {
     const Geometry& g = a.g;
-    const int64_t cell = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const int64_t n_cells = (int64_t)g.n_gu * g.n_strips;
-    const int lane = threadIdx.x & 31, warp = (threadIdx.x >> 5) & 7;
-    if (cell > n_cells) return;
-    if (cell == n_cells) {                                   // terminator of the exclusive scans
-        if (MODE == 0 && lane == 0) hits[cell] = items[cell] = 0;
-        return;
-    }
-    const int gu = (int)(cell / g.n_strips), strip = (int)(cell - (int64_t)gu * g.n_strips);
-    const int kset = a.gu_set[gu];
-    const SetPlan sp = a.set_plan[kset];
-    const int S = a.set_support[kset], h_lo = S / 2;
-    const int sub_lo = (gu - sp.gu_base) * sp.group_slices;
-    int Xw, Yw, bx_lo, bx_hi, by_lo, by_hi;
-    strip_buckets(g, strip, S, Xw, Yw, bx_lo, bx_hi, by_lo, by_hi);
-    int out = 0;
-    if (MODE == 1) {
-        out = hits[cell];
-        const int n_hits = hits[cell + 1] - out;
-        if (n_hits == 0) return;
-        const int i0 = items[cell], n_items = items[cell + 1] - i0;
-        for (int p = lane; p < n_items; p += 32)
-            item_rec[i0 + p] = Item{strip, out + p * kItemHits, min(kItemHits, n_hits - p * kItemHits), gu};
-        for (int v = lane; v < 128; v += 32) s_bin[warp][v] = 0;
-        __syncwarp();
-    }
-    const int slice_taps = sp.rows * sp.pitch;
-    const unsigned lt_mask = (1u << lane) - 1u;
-    int count = 0;
-    // pass 0: count (MODE 0) or histogram by variant (MODE 1); pass 1 (MODE 1 only): stable scatter
-    for (int pass = 0; pass <= MODE; ++pass) {
-        if (pass == 1) {                                     // exclusive prefix of the 108 bins, 4 per lane
-            __syncwarp();
-            int c[4], t = 0;
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                c[q] = s_bin[warp][4 * lane + q];
-                t += c[q];
-            }
-            int inc = t;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const int y = __shfl_up_sync(0xffffffffu, inc, d);
-                if (lane >= d) inc += y;
-            }
-            int run = inc - t;
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                s_bin[warp][4 * lane + q] = run;
-                run += c[q];
-            }
-            __syncwarp();
-        }
-        for (int by = by_lo; by <= by_hi; ++by) {
-            const int b0 = (kset * g.nt + by) * g.nt;
-            const int r0 = a.bucket_offset[b0 + bx_lo], r1 = a.bucket_offset[b0 + bx_hi + 1];
-            for (int i0 = r0; i0 < r1; i0 += 32) {
-                const int idx = i0 + lane;
-                uint32_t ctrl = 0u;
-                int dx0 = 0, dy0 = 0, sub = 0;
-                if (idx < r1) {
-                    const uint2 geo = a.sgeo[idx];
-                    const int gx = (int)(geo.x & 0xffffu), gy = (int)(geo.x >> 16);
-                    dx0 = Xw - (gx - h_lo);                                  // tap coordinates of the strip origin
-                    dy0 = Yw - (gy - h_lo);
-                    sub = (int)geo.y - sub_lo;
-                    ctrl = hit_ctrl(dx0, dy0, S, sub, sp.group_slices);
-                }
-                const unsigned m = __ballot_sync(0xffffffffu, ctrl != 0u);
-                if (MODE == 0) {
-                    count += __popc(m);
-                } else if (m) {
-                    const uint32_t v = ctrl ? ctrl_variant(ctrl) : 127u;
-                    if (pass == 0) {
-                        if (ctrl) atomicAdd(&s_bin[warp][v], 1);
-                    } else {
-                        const unsigned peers = __match_any_sync(0xffffffffu, v);
-                        const int leader = __ffs(peers) - 1, rank = __popc(peers & lt_mask);
-                        int base = 0;
-                        if (lane == leader && ctrl) {
-                            base = s_bin[warp][v];
-                            s_bin[warp][v] = base + __popc(peers);
-                        }
-                        base = __shfl_sync(0xffffffffu, base, leader);
-                        if (ctrl) {
-                            const int tapoff = sub * slice_taps + (dy0 + kPadY) * sp.pitch + dx0 + kPadX;
-                            hit_rec[out + base + rank] = make_uint2((uint32_t)idx, (uint32_t)(tapoff + (int)kTapBias) | (ctrl << 24));
-                        }
-                    }
-                }
-            }
-        }
-    }
-    if (MODE == 0 && lane == 0) {
-        hits[cell] = count;
-        items[cell] = (count + kItemHits - 1) / kItemHits;
+    const int n_kept = counters[0];
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_kept; i += gridDim.x * blockDim.x) {
+        const uint2 geo = a.sgeo[i];
+        const int gx = (int)(geo.x & 0xffffu), gy = (int)(geo.x >> 16);
+        const int sub = (int)(geo.y & kSubMask), kset = (int)(geo.y >> kSubBits);
+        const SetPlan sp = a.set_plan[kset];
+        const int S = a.set_support[kset], h_lo = S / 2;
+        const int gu = sp.gu_base + sub / sp.group_slices;
+        const int x0 = gx - h_lo, y0 = gy - h_lo;                       // footprint origin, inside the grid for kept ones
+        const int sx0 = x0 / kStripW, sx1 = (x0 + S - 1) / kStripW, sy0 = y0 / kStripH, sy1 = (y0 + S - 1) / kStripH;
+        int32_t* base = hits + (int64_t)gu * g.n_strips;
+        for (int sy = sy0; sy <= sy1; ++sy)
+            for (int sx = sx0; sx <= sx1; ++sx) atomicAdd(base + sy * g.strips_per_row + sx, 1);
     }
 }
 
-// one thread block: per geometry unit, blocks of about kBlockHits hits (whole items), replicated for every Mueller
+// items[cell] = ceil(hits[cell] / kItemHits); entry n_cells (the terminator of the exclusive scans) is 0 in both
+__global__ void items_from_hits_kernel(int64_t n_cells, const int32_t* __restrict__ hits, int32_t* __restrict__ items) {
+    for (int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; c <= n_cells; c += (int64_t)gridDim.x * blockDim.x)
+        items[c] = c < n_cells ? (hits[c] + kItemHits - 1) / kItemHits : 0;
+}
+
+// Unsorted hit records, visibility-centric: the same enumeration as count_hits_kernel; a hit takes the next free place
+// of its cell's range (hit_start[cell] + cursor[cell]++).
+__global__ void emit_hits_kernel(const PlanArgs a, const int32_t* __restrict__ counters, const int32_t* __restrict__ hit_start,
+                                 int32_t* __restrict__ cursor, uint2* __restrict__ hit_tmp) {
+    const Geometry& g = a.g;
+    const int n_kept = counters[0];
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_kept; i += gridDim.x * blockDim.x) {
+        const uint2 geo = a.sgeo[i];
+        const int gx = (int)(geo.x & 0xffffu), gy = (int)(geo.x >> 16);
+        const int sub = (int)(geo.y & kSubMask), kset = (int)(geo.y >> kSubBits);
+        const SetPlan sp = a.set_plan[kset];
+        const int S = a.set_support[kset], h_lo = S / 2;
+        const int group = sub / sp.group_slices, subl = sub - group * sp.group_slices;
+        const int gu = sp.gu_base + group;
+        const int x0 = gx - h_lo, y0 = gy - h_lo;
+        const int sx0 = x0 / kStripW, sx1 = (x0 + S - 1) / kStripW, sy0 = y0 / kStripH, sy1 = (y0 + S - 1) / kStripH;
+        const int slice_taps = sp.rows * sp.pitch;
+        for (int sy = sy0; sy <= sy1; ++sy)
+            for (int sx = sx0; sx <= sx1; ++sx) {
+                const int dx0 = sx * kStripW - x0, dy0 = sy * kStripH - y0;      // tap coordinates of the strip origin
+                const uint32_t ctrl = hit_ctrl(dx0, dy0, S, subl, sp.group_slices);
+                const int64_t cell = (int64_t)gu * g.n_strips + sy * g.strips_per_row + sx;
+                const int pos = atomicAdd(cursor + cell, 1);
+                const int tapoff = subl * slice_taps + (dy0 + kPadY) * sp.pitch + dx0 + kPadX;
+                hit_tmp[(int64_t)hit_start[cell] + pos] = make_uint2((uint32_t)i, (uint32_t)(tapoff + (int)kTapBias) | (ctrl << 24));
+            }
+    }
+}
+
+// One warp per (gu, strip): counting sort of the cell's hit records by variant (hit_tmp -> hit_rec), so that the
+// kernels replay runs of hits with the same slot range, and the cell's item records.
+__global__ void __launch_bounds__(256) sort_hits_kernel(const Geometry g, const int32_t* __restrict__ hits,
+                                                        const int32_t* __restrict__ items, const uint2* __restrict__ hit_tmp,
+                                                        uint2* __restrict__ hit_rec, Item* __restrict__ item_rec) {
+    __shared__ int32_t s_bin[8][128];
+    const int64_t cell = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int64_t n_cells = (int64_t)g.n_gu * g.n_strips;
+    const int lane = threadIdx.x & 31, warp = (threadIdx.x >> 5) & 7;
+    if (cell >= n_cells) return;
+    const int out = hits[cell], n_hits = hits[cell + 1] - out;
+    if (n_hits == 0) return;
+    const int gu = (int)(cell / g.n_strips), strip = (int)(cell - (int64_t)gu * g.n_strips);
+    const int i0 = items[cell], n_items = items[cell + 1] - i0;
+    for (int p = lane; p < n_items; p += 32)
+        item_rec[i0 + p] = Item{strip, out + p * kItemHits, min(kItemHits, n_hits - p * kItemHits), gu};
+    for (int v = lane; v < 128; v += 32) s_bin[warp][v] = 0;
+    __syncwarp();
+    for (int q = lane; q < n_hits; q += 32) atomicAdd(&s_bin[warp][ctrl_variant(hit_tmp[out + q].y >> 24)], 1);
+    __syncwarp();
+    {                                                          // exclusive prefix of the 108 bins, 4 per lane
+        int c[4], t = 0;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            c[q] = s_bin[warp][4 * lane + q];
+            t += c[q];
+        }
+        int inc = t;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int y = __shfl_up_sync(0xffffffffu, inc, d);
+            if (lane >= d) inc += y;
+        }
+        int run = inc - t;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            s_bin[warp][4 * lane + q] = run;
+            run += c[q];
+        }
+    }
+    __syncwarp();
+    const unsigned lt_mask = (1u << lane) - 1u;
+    for (int q0 = 0; q0 < n_hits; q0 += 32) {
+        const bool have = q0 + lane < n_hits;
+        uint2 r = make_uint2(0u, 0u);
+        if (have) r = hit_tmp[out + q0 + lane];
+        const uint32_t v = have ? ctrl_variant(r.y >> 24) : 127u;
+        const unsigned peers = __match_any_sync(0xffffffffu, v);
+        const int leader = __ffs(peers) - 1, rank = __popc(peers & lt_mask);
+        int base = 0;
+        if (lane == leader && have) {
+            base = s_bin[warp][v];
+            s_bin[warp][v] = base + __popc(peers);
+        }
+        base = __shfl_sync(0xffffffffu, base, leader);
+        if (have) hit_rec[out + base + rank] = r;
+        __syncwarp();
+    }
+}
+
+// one thread block per geometry unit: blocks of about kBlockHits hits (whole items), replicated for every Mueller
 // element sc = s * n_corr + c.  Block order is irrelevant (a work queue consumes them).
 __global__ void plan_blocks_kernel(const Geometry g, const int32_t* __restrict__ hit_start, const int32_t* __restrict__ item_start,
                                    const Item* __restrict__ item_rec, Block* __restrict__ blocks, int32_t* __restrict__ n_blocks,
                                    int max_blocks) {
-    __shared__ int s_total;
-    if (threadIdx.x == 0) s_total = 0;
-    __syncthreads();
+    __shared__ int s_base;
+    const int gu = blockIdx.x;
     const int n_sc = g.n_pol * g.n_corr;
-    for (int gu = threadIdx.x; gu < g.n_gu; gu += blockDim.x) {
-        const int64_t c0 = (int64_t)gu * g.n_strips, c1 = c0 + g.n_strips;
-        const int h0 = hit_start[c0], h1 = hit_start[c1], i0 = item_start[c0], i1 = item_start[c1];
-        if (h1 == h0) continue;
-        const int nb = (h1 - h0 + kBlockHits - 1) / kBlockHits;
-        const int base = atomicAdd(&s_total, nb * n_sc);
-        if (base + nb * n_sc > max_blocks) continue;                      // cannot happen: max_blocks is an upper bound
-        int first = i0;
-        for (int b = 0; b < nb; ++b) {
-            // first item whose hit_begin >= h0 + (b + 1) * kBlockHits
-            const int limit = h0 + (b + 1) * kBlockHits;
-            int lo = first, hi = i1;
+    const int64_t c0 = (int64_t)gu * g.n_strips, c1 = c0 + g.n_strips;
+    const int h0 = hit_start[c0], h1 = hit_start[c1], i0 = item_start[c0], i1 = item_start[c1];
+    if (h1 == h0) return;
+    const int nb = (h1 - h0 + kBlockHits - 1) / kBlockHits;
+    if (threadIdx.x == 0) s_base = atomicAdd(n_blocks, nb * n_sc);
+    __syncthreads();
+    const int base = s_base;
+    if (base + nb * n_sc > max_blocks) return;                        // cannot happen: max_blocks is an upper bound
+    for (int b = threadIdx.x; b < nb; b += blockDim.x) {
+        int bounds[2];                                                // items [first, last): hit_begin in [h0 + b K, h0 + (b + 1) K)
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const int64_t limit = (int64_t)h0 + (int64_t)(b + e) * kBlockHits;
+            int lo = i0, hi = i1;
             while (lo < hi) {
                 const int mid = (lo + hi) >> 1;
                 if (item_rec[mid].hit_begin < limit) lo = mid + 1; else hi = mid;
             }
-            const int last = (b == nb - 1) ? i1 : lo;
-            for (int sc = 0; sc < n_sc; ++sc) blocks[base + sc * nb + b] = Block{gu, sc, first, last - first};
-            first = last;
+            bounds[e] = lo;
         }
+        if (b == nb - 1) bounds[1] = i1;
+        for (int sc = 0; sc < n_sc; ++sc) blocks[base + sc * nb + b] = Block{gu, sc, bounds[0], bounds[1] - bounds[0]};
     }
-    __syncthreads();
-    if (threadIdx.x == 0) *n_blocks = min(s_total, max_blocks);
 }
 
 // ---- the kernels -----------------------------------------------------------------------------------------
@@ -721,9 +732,11 @@ struct TiledState {
     int32_t* d_items = nullptr;           // [n_cells + 1] -> scanned into item starts
     int32_t* d_scan_tmp = nullptr;
     uint2* d_hit_rec = nullptr;
+    uint2* d_hit_tmp = nullptr;           // unsorted hit records (planner scratch)
+    int32_t* d_cursor = nullptr;          // [n_cells + 1] fill cursors of emit_hits_kernel
     Item* d_item_rec = nullptr;
     Block* d_blocks = nullptr;
-    int64_t cap_hits = 0, cap_items = 0, cap_blocks = 0;
+    int64_t cap_hits = 0, cap_items = 0, cap_blocks = 0, cap_tmp = 0;
     int32_t* h_totals = nullptr;          // pinned [2]
     uint2* d_sgeo = nullptr;
     float2* d_sval = nullptr;
@@ -734,7 +747,7 @@ struct TiledState {
 
 bool tiled_supported(const imager_plan* pl) {
     const imager_params& p = pl->p;
-    if (p.grid_size % kStripH != 0 || p.grid_size > 32768) return false;
+    if (p.grid_size % kStripH != 0 || p.grid_size > 32768 || pl->n_sets >= (1 << (32 - kSubBits))) return false;
     // every slice (with its padding) must fit in shared memory, and the planner enumerates (gu, strip) pairs
     const int64_t n_strips = (int64_t)(p.grid_size / kStripW) * (p.grid_size / kStripH);
     int64_t n_gu = 0;
@@ -797,6 +810,8 @@ void tiled_release(imager_plan* pl) {
     cudaFree(st->d_items);
     cudaFree(st->d_scan_tmp);
     cudaFree(st->d_hit_rec);
+    cudaFree(st->d_hit_tmp);
+    cudaFree(st->d_cursor);
     cudaFree(st->d_item_rec);
     cudaFree(st->d_blocks);
     cudaFree(st->d_sgeo);
@@ -834,6 +849,7 @@ static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
         for (int64_t n = n_cells + 1; n > 1; n = (n + 1023) / 1024) tmp_len += (n + 1023) / 1024 + 1;
         IMAGER_CUDA(cudaMalloc(&st->d_hits, (n_cells + 1) * sizeof(int32_t)));
         IMAGER_CUDA(cudaMalloc(&st->d_items, (n_cells + 1) * sizeof(int32_t)));
+        IMAGER_CUDA(cudaMalloc(&st->d_cursor, (n_cells + 1) * sizeof(int32_t)));
         IMAGER_CUDA(cudaMalloc(&st->d_scan_tmp, tmp_len * sizeof(int32_t)));
         IMAGER_CUDA(cudaMalloc(&st->d_sgeo, mv * sizeof(uint2)));
         IMAGER_CUDA(cudaMalloc(&st->d_sval, mv * pl->p.n_corr * sizeof(float2)));
@@ -854,8 +870,10 @@ static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
     pa.bucket_offset = pl->d_bucket_offset;
     pa.sgeo = st->d_sgeo;
     const unsigned nb = (unsigned)((n_cells + 1 + 7) / 8);               // 8 warps per thread block
-    plan_hits_kernel<0><<<nb, 256, 0, stream>>>(pa, st->d_hits, st->d_items, nullptr, nullptr);
-    pl->last_launches += 2;
+    IMAGER_CUDA(cudaMemsetAsync(st->d_hits, 0, (n_cells + 1) * sizeof(int32_t), stream));
+    count_hits_kernel<<<8 * kNumSMs, 256, 0, stream>>>(pa, pl->d_counters, st->d_hits);
+    items_from_hits_kernel<<<2 * kNumSMs, 256, 0, stream>>>(n_cells, st->d_hits, st->d_items);
+    pl->last_launches += 3;
     int rc = exclusive_scan_i32(pl, st->d_hits, n_cells + 1, st->d_scan_tmp, stream);
     if (rc) return rc;
     rc = exclusive_scan_i32(pl, st->d_items, n_cells + 1, st->d_scan_tmp, stream);
@@ -876,9 +894,15 @@ static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
     if (rc) return rc;
     rc = grow(&st->d_blocks, &st->cap_blocks, max_blocks + 1);
     if (rc) return rc;
-    plan_hits_kernel<1><<<nb, 256, 0, stream>>>(pa, st->d_hits, st->d_items, st->d_hit_rec, st->d_item_rec);
-    plan_blocks_kernel<<<1, 1024, 0, stream>>>(g, st->d_hits, st->d_items, st->d_item_rec, st->d_blocks, pl->d_counters + 9,
-                                               (int)std::min<int64_t>(st->cap_blocks, 0x7fffffff));
+    rc = grow(&st->d_hit_tmp, &st->cap_tmp, n_hits + 1);
+    if (rc) return rc;
+    IMAGER_CUDA(cudaMemsetAsync(st->d_cursor, 0, (n_cells + 1) * sizeof(int32_t), stream));
+    emit_hits_kernel<<<8 * kNumSMs, 256, 0, stream>>>(pa, pl->d_counters, st->d_hits, st->d_cursor, st->d_hit_tmp);
+    sort_hits_kernel<<<nb, 256, 0, stream>>>(g, st->d_hits, st->d_items, st->d_hit_tmp, st->d_hit_rec, st->d_item_rec);
+    pl->last_launches += 1;
+    IMAGER_CUDA(cudaMemsetAsync(pl->d_counters + 9, 0, sizeof(int32_t), stream));
+    plan_blocks_kernel<<<g.n_gu, 128, 0, stream>>>(g, st->d_hits, st->d_items, st->d_item_rec, st->d_blocks, pl->d_counters + 9,
+                                                   (int)std::min<int64_t>(st->cap_blocks, 0x7fffffff));
     pl->last_launches += 2;
     IMAGER_CUDA(cudaGetLastError());
     st->plan_epoch = pl->index_epoch;
