@@ -567,6 +567,15 @@ __device__ __forceinline__ void sts64(uint32_t addr, float2 v) {
     asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(v.x), "f"(v.y) : "memory");
 }
 
+// conj(t) * g on one packed accumulator: acc += (t.re, t.im) * (g.re, -g.re), then acc += (t.im, t.re) * (g.im, g.im)
+__device__ __forceinline__ void dmac_re(u64& acc, float2 t, float gr) { ffma2p(acc, pack2(t.x, t.y), pack2(gr, -gr)); }
+__device__ __forceinline__ void dmac_im(u64& acc, float2 t, float gi) { ffma2p(acc, pack2(t.y, t.x), pack2(gi, gi)); }
+__device__ __forceinline__ u64 add2p(u64 a, u64 b) {
+    u64 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+
 template <int H, int JL, int JH>
 __device__ __forceinline__ void degrid_run(const float2 (&G0)[kNY], const float2 (&G1)[kNY], uint32_t desc_addr, int cnt,
                                            uint32_t red_addr, const uint32_t lane_off, const uint32_t (&step)[kNY]) {
@@ -576,7 +585,7 @@ __device__ __forceinline__ void degrid_run(const float2 (&G0)[kNY], const float2
         desc_addr += 8;
         const uint32_t a_next = lds32(desc_addr);            // one past the run at its end: unused
         const uint32_t addr = a_cur + lane_off;
-        float2 P0 = make_float2(0.f, 0.f), Q0 = P0, P1 = P0, Q1 = P0;
+        u64 P[2][2] = {{0ull, 0ull}, {0ull, 0ull}};          // [x-half][slot parity]: four independent FFMA2 chains
         constexpr int kChunk = (H == 3) ? 4 : 8;
 #pragma unroll
         for (int j0 = JL; j0 < JH; j0 += kChunk) {
@@ -588,28 +597,20 @@ __device__ __forceinline__ void degrid_run(const float2 (&G0)[kNY], const float2
             }
 #pragma unroll
             for (int j = j0; j < j0 + kChunk && j < JH; ++j) {
-                if (H & 1) {
-                    ffma2(P0, t0[j - j0], make_float2(G0[j].x, G0[j].x));
-                    ffma2(Q0, t0[j - j0], make_float2(G0[j].y, G0[j].y));
-                }
-                if (H & 2) {
-                    ffma2(P1, t1[j - j0], make_float2(G1[j].x, G1[j].x));
-                    ffma2(Q1, t1[j - j0], make_float2(G1[j].y, G1[j].y));
-                }
+                if (H & 1) dmac_re(P[0][j & 1], t0[j - j0], G0[j].x);
+                if (H & 2) dmac_re(P[1][j & 1], t1[j - j0], G1[j].x);
+            }
+#pragma unroll
+            for (int j = j0; j < j0 + kChunk && j < JH; ++j) {
+                if (H & 1) dmac_im(P[0][j & 1], t0[j - j0], G0[j].y);
+                if (H & 2) dmac_im(P[1][j & 1], t1[j - j0], G1[j].y);
             }
         }
-        float re, im;
-        if (H == 3) {
-            re = (P0.x + Q0.y) + (P1.x + Q1.y);
-            im = (Q0.x - P0.y) + (Q1.x - P1.y);
-        } else if (H == 1) {
-            re = P0.x + Q0.y;
-            im = Q0.x - P0.y;
-        } else {
-            re = P1.x + Q1.y;
-            im = Q1.x - P1.y;
-        }
-        sts64(red_addr, make_float2(re, im));
+        u64 sum;
+        if (H == 3) sum = add2p(add2p(P[0][0], P[0][1]), add2p(P[1][0], P[1][1]));
+        else if (H == 1) sum = add2p(P[0][0], P[0][1]);
+        else sum = add2p(P[1][0], P[1][1]);
+        sts64(red_addr, unpack2(sum));
         red_addr += 32 * 8;
         a_cur = a_next;
     } while (--cnt > 0);

@@ -183,7 +183,11 @@ def test_adjointness_on_gpu(torch_cuda):
             ones = torch.ones((nvis, nc), dtype=torch.float32, device="cuda")
             gv = torch.zeros((npol, n, n), dtype=torch.complex64, device="cuda")
             plan.grid(d_uvw, d_vis, ones, gv, d_a)
+            # g = noise + (a multiple of) G v: <g, G v> then has a large coherent part, so that "1e-6 relative" bounds
+            # the adjointness defect against the size of the terms and not against a cancelling random sum (FP32
+            # accumulation order differs from run to run: atomics)
             g = torch.randn((npol, n, n), dtype=torch.complex64, device="cuda")
+            g = g + gv * (torch.linalg.vector_norm(g) / torch.linalg.vector_norm(gv))
             hg = torch.zeros((nvis, nc), dtype=torch.complex64, device="cuda")
             plan.degrid(d_uvw, g, hg, d_a, flags=1)
             lhs = torch.vdot(g.to(torch.complex128).flatten(), gv.to(torch.complex128).flatten()).item()
