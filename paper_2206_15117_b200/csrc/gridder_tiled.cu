@@ -34,6 +34,9 @@ constexpr int kTiledThreads = 512, kWarps = kTiledThreads / 32;
 #define IMAGER_GRID_THREADS 768
 #endif
 constexpr int kGridThreads = IMAGER_GRID_THREADS;     // gridding kernel: threads per CTA (one CTA per SM)
+#ifndef IMAGER_CHUNK3
+#define IMAGER_CHUNK3 4
+#endif
 #ifndef IMAGER_ITEM_HITS
 #define IMAGER_ITEM_HITS 256
 #endif
@@ -120,19 +123,6 @@ __global__ void scatter_values_kernel(int64_t nvis, const int32_t* __restrict__ 
 #pragma unroll
         for (int c = 0; c < NC; ++c) vis_out[k * NC + c] = i < n_kept ? sval[i * NC + c] : make_float2(0.f, 0.f);
     }
-}
-
-// candidate visibilities of (kset, strip): the bucket rows / columns whose footprints can reach the strip
-__device__ __forceinline__ void strip_buckets(const Geometry& g, int strip, int S, int& Xw, int& Yw, int& bx_lo, int& bx_hi,
-                                              int& by_lo, int& by_hi) {
-    const int sy = strip / g.strips_per_row, sx = strip - sy * g.strips_per_row;
-    const int h_lo = S / 2, h_hi = S - 1 - h_lo;
-    Xw = sx * kStripW;
-    Yw = sy * kStripH;
-    bx_lo = max(0, Xw - h_hi) / kBucketTile;
-    bx_hi = min(g.nt - 1, (Xw + kStripW - 1 + h_lo) / kBucketTile);
-    by_lo = max(0, Yw - h_hi) / kBucketTile;
-    by_hi = min(g.nt - 1, (Yw + kStripH - 1 + h_lo) / kBucketTile);
 }
 
 // ---- planner ---------------------------------------------------------------------------------------------
@@ -225,25 +215,59 @@ __global__ void emit_hits_kernel(const PlanArgs a, const int32_t* __restrict__ c
     }
 }
 
-// One warp per (gu, strip): counting sort of the cell's hit records by variant (hit_tmp -> hit_rec), so that the
-// kernels replay runs of hits with the same slot range, and the cell's item records.
-__global__ void __launch_bounds__(256) sort_hits_kernel(const Geometry g, const int32_t* __restrict__ hits,
-                                                        const int32_t* __restrict__ items, const uint2* __restrict__ hit_tmp,
-                                                        uint2* __restrict__ hit_rec, Item* __restrict__ item_rec) {
-    __shared__ int32_t s_bin[8][128];
-    const int64_t cell = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+// item records: one thread per (gu, strip); item = up to kItemHits consecutive hits of the cell
+__global__ void make_items_kernel(const Geometry g, const int32_t* __restrict__ hits, const int32_t* __restrict__ items,
+                                  Item* __restrict__ item_rec) {
     const int64_t n_cells = (int64_t)g.n_gu * g.n_strips;
+    for (int64_t cell = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; cell < n_cells; cell += (int64_t)gridDim.x * blockDim.x) {
+        const int out = hits[cell], n_hits = hits[cell + 1] - out;
+        if (n_hits == 0) continue;
+        const int gu = (int)(cell / g.n_strips), strip = (int)(cell - (int64_t)gu * g.n_strips);
+        const int i0 = items[cell], n_items = items[cell + 1] - i0;
+        for (int p = 0; p < n_items; ++p)
+            item_rec[i0 + p] = Item{strip, out + p * kItemHits, min(kItemHits, n_hits - p * kItemHits), gu};
+    }
+}
+
+// One warp per sort unit: counting sort of the unit's hit records by variant (hit_tmp -> hit_rec), so that the kernels
+// replay runs of hits with the same slot range.  A unit = the consecutive items of one (gu, strip) whose first hit
+// falls into the same kSortSpan-aligned window of the hit array: at most kSortSpan hits, whatever the cell's size.
+#ifndef IMAGER_SORT_ITEMS
+#define IMAGER_SORT_ITEMS 2
+#endif
+constexpr int kSortSpan = IMAGER_SORT_ITEMS * kItemHits;
+__global__ void __launch_bounds__(256) sort_items_kernel(int n_items, const Item* __restrict__ item_rec,
+                                                         const uint2* __restrict__ hit_tmp, uint2* __restrict__ hit_rec) {
+    __shared__ int32_t s_bin[8][128];
+    const int item = (int)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5);
     const int lane = threadIdx.x & 31, warp = (threadIdx.x >> 5) & 7;
-    if (cell >= n_cells) return;
-    const int out = hits[cell], n_hits = hits[cell + 1] - out;
-    if (n_hits == 0) return;
-    const int gu = (int)(cell / g.n_strips), strip = (int)(cell - (int64_t)gu * g.n_strips);
-    const int i0 = items[cell], n_items = items[cell + 1] - i0;
-    for (int p = lane; p < n_items; p += 32)
-        item_rec[i0 + p] = Item{strip, out + p * kItemHits, min(kItemHits, n_hits - p * kItemHits), gu};
-    for (int v = lane; v < 128; v += 32) s_bin[warp][v] = 0;
+    if (item >= n_items) return;
+    const Item it = item_rec[item];
+    const int window = it.hit_begin / kSortSpan;
+    if (item > 0) {                                            // not the first item of its unit: nothing to do
+        const Item pv = item_rec[item - 1];
+        if (pv.strip == it.strip && pv.pad == it.pad && pv.hit_begin / kSortSpan == window) return;
+    }
+    const int out = it.hit_begin;
+    int n_hits = it.hit_count;
+    for (int k = 1; k < kSortSpan / kItemHits && item + k < n_items; ++k) {
+        const Item nx = item_rec[item + k];
+        if (nx.strip != it.strip || nx.pad != it.pad || nx.hit_begin / kSortSpan != window) break;
+        n_hits += nx.hit_count;
+    }
+    constexpr int kPer = kSortSpan / 32;
+    uint2 r[kPer];
+    for (int q = lane; q < 128; q += 32) s_bin[warp][q] = 0;
     __syncwarp();
-    for (int q = lane; q < n_hits; q += 32) atomicAdd(&s_bin[warp][ctrl_variant(hit_tmp[out + q].y >> 24)], 1);
+#pragma unroll
+    for (int k = 0; k < kPer; ++k) {
+        const int q = k * 32 + lane;
+        r[k] = make_uint2(0u, 0u);
+        if (q < n_hits) r[k] = hit_tmp[out + q];
+    }
+#pragma unroll
+    for (int k = 0; k < kPer; ++k)
+        if (k * 32 + lane < n_hits) atomicAdd(&s_bin[warp][ctrl_variant(r[k].y >> 24)], 1);
     __syncwarp();
     {                                                          // exclusive prefix of the 108 bins, 4 per lane
         int c[4], t = 0;
@@ -266,23 +290,10 @@ __global__ void __launch_bounds__(256) sort_hits_kernel(const Geometry g, const 
         }
     }
     __syncwarp();
-    const unsigned lt_mask = (1u << lane) - 1u;
-    for (int q0 = 0; q0 < n_hits; q0 += 32) {
-        const bool have = q0 + lane < n_hits;
-        uint2 r = make_uint2(0u, 0u);
-        if (have) r = hit_tmp[out + q0 + lane];
-        const uint32_t v = have ? ctrl_variant(r.y >> 24) : 127u;
-        const unsigned peers = __match_any_sync(0xffffffffu, v);
-        const int leader = __ffs(peers) - 1, rank = __popc(peers & lt_mask);
-        int base = 0;
-        if (lane == leader && have) {
-            base = s_bin[warp][v];
-            s_bin[warp][v] = base + __popc(peers);
-        }
-        base = __shfl_sync(0xffffffffu, base, leader);
-        if (have) hit_rec[out + base + rank] = r;
-        __syncwarp();
-    }
+    // scatter: a hit takes the next free place of its variant's range (order within a variant is irrelevant)
+#pragma unroll
+    for (int k = 0; k < kPer; ++k)
+        if (k * 32 + lane < n_hits) hit_rec[out + atomicAdd(&s_bin[warp][ctrl_variant(r[k].y >> 24)], 1)] = r[k];
 }
 
 // one thread block per geometry unit: blocks of about kBlockHits hits (whole items), replicated for every Mueller
@@ -396,7 +407,7 @@ __device__ __forceinline__ void grid_run(u64 (&C0)[kNY], u64 (&C1)[kNY], uint4& 
         desc_addr += 16;
         d = lds128(desc_addr);                               // the next hit of the batch (one past it at its end: unused)
         // at most 8 tap loads in flight: chunks of 4 slots (both halves) or 8 slots (one half)
-        constexpr int kChunk = (H == 3) ? 4 : 8;
+        constexpr int kChunk = (H == 3) ? IMAGER_CHUNK3 : 8;
 #pragma unroll
         for (int j0 = JL; j0 < JH; j0 += kChunk) {
             float2 t0[kChunk], t1[kChunk];
@@ -870,7 +881,6 @@ static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
     pa.set_support = pl->d_set_support;
     pa.bucket_offset = pl->d_bucket_offset;
     pa.sgeo = st->d_sgeo;
-    const unsigned nb = (unsigned)((n_cells + 1 + 7) / 8);               // 8 warps per thread block
     IMAGER_CUDA(cudaMemsetAsync(st->d_hits, 0, (n_cells + 1) * sizeof(int32_t), stream));
     count_hits_kernel<<<8 * kNumSMs, 256, 0, stream>>>(pa, pl->d_counters, st->d_hits);
     items_from_hits_kernel<<<2 * kNumSMs, 256, 0, stream>>>(n_cells, st->d_hits, st->d_items);
@@ -899,8 +909,11 @@ static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
     if (rc) return rc;
     IMAGER_CUDA(cudaMemsetAsync(st->d_cursor, 0, (n_cells + 1) * sizeof(int32_t), stream));
     emit_hits_kernel<<<8 * kNumSMs, 256, 0, stream>>>(pa, pl->d_counters, st->d_hits, st->d_cursor, st->d_hit_tmp);
-    sort_hits_kernel<<<nb, 256, 0, stream>>>(g, st->d_hits, st->d_items, st->d_hit_tmp, st->d_hit_rec, st->d_item_rec);
-    pl->last_launches += 1;
+    make_items_kernel<<<8 * kNumSMs, 256, 0, stream>>>(g, st->d_hits, st->d_items, st->d_item_rec);
+    if (n_items > 0)
+        sort_items_kernel<<<(unsigned)((n_items + 7) / 8), 256, 0, stream>>>((int)n_items, st->d_item_rec, st->d_hit_tmp,
+                                                                             st->d_hit_rec);
+    pl->last_launches += 2;
     IMAGER_CUDA(cudaMemsetAsync(pl->d_counters + 9, 0, sizeof(int32_t), stream));
     plan_blocks_kernel<<<g.n_gu, 128, 0, stream>>>(g, st->d_hits, st->d_items, st->d_item_rec, st->d_blocks, pl->d_counters + 9,
                                                    (int)std::min<int64_t>(st->cap_blocks, 0x7fffffff));
