@@ -48,13 +48,19 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-def build_probe() -> str:
-    """The operand-port micro-benchmarks quoted in DESIGN.md / profiles/r1_port_probe.md (a standalone executable)."""
+PROBES = ["port_probe", "lds_mask_probe", "tmem_shape_probe"]
+
+
+def build_probe() -> list:
+    """The micro-benchmarks quoted in DESIGN.md / profiles/r1_*_probe.md (standalone executables next to the library)."""
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    exe = os.path.join(HERE, "port_probe")
-    subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
-                           os.path.join(CSRC, "port_probe.cu"), "-o", exe])
-    return exe
+    out = []
+    for name in PROBES:
+        exe = os.path.join(HERE, name)
+        subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
+                               os.path.join(CSRC, name + ".cu"), "-o", exe])
+        out.append(exe)
+    return out
 
 
 if __name__ == "__main__":
