@@ -241,10 +241,12 @@ def run_ours(args):
     value = world * nvis / (ms_per_step * 1e-3)
     peak_tflops = N_SM * FP32_FMA_PER_CLK_SM * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 * 2 / 1e12
     achieved = 8.0 * cmacs / (kern["grid"] * 1e-3) / 1e12
-    traffic = None
-    prof = os.path.join(ROOT, "profiles", "traffic_bytes.json")
-    if os.path.exists(prof):
-        traffic = json.load(open(prof)).get("grid_kernel_dram_bytes_per_launch")
+    traffic = None                                  # DRAM bytes per launch of the gridding kernel, from the committed ncu capture
+    prof = os.path.join(ROOT, "profiles", "r1b_traffic.txt")
+    if os.path.exists(prof) and args.workload == "config2" and args.time_stride == 1:
+        for ln in open(prof):
+            if ln.startswith("grid_kernel_dram_bytes_per_launch"):
+                traffic = int(ln.split()[1])
     line = {
         "metric": "visibilities gridded+degridded/sec", "value": value, "unit": "vis/s", "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
