@@ -126,6 +126,14 @@ int imager_plan_destroy(imager_plan* plan);
  * psi psi, then the centred unnormalised inverse DFT (R1: signs follow Eq. 2).  data dev complex64. */
 int imager_grid_image_transform(imager_plan* plan, float* data, int32_t direction, double norm, void* cuda_stream);
 
+/* UV-domain mosaic weighting correction, Eq. 1: multiplies every [N][N] plane of `image` (dev complex64
+ * [n_pol][N][N], pixel (N/2, N/2) at l = m = 0, the output of imager_grid_image_transform(+1)) in place by
+ * gamma(l,m) = [sqrt(sum_i B_i^2) / max sqrt(sum_i B_i^2)] * [1 / sum_i B_i^2], B_i(l,m) = E^2(l - l_i, m - m_i) the
+ * power beam of pointing i (the gridding kernel of MOSAIC_PB mode; E the Airy pattern of dish_diameter_m at freq_hz).
+ * gamma is built on the device at the first call and cached in the plan.  Errors: INVALID_ARG (NULL, plan not in
+ * MOSAIC_PB mode), NOMEM, CUDA. */
+int imager_mosaic_correct(imager_plan* plan, float* image, void* cuda_stream);
+
 /* ---- test / debug exports (synchronise; not part of the hot path) ---- */
 
 /* Runs indexing + bucketing for (uvw, a_index) and copies out: records host [nvis], perm host int32 [nvis]

@@ -22,7 +22,7 @@ PATH_SMEM = 4
 PATH_TMEM = 8
 
 EXPORTS = ("imager_plan_create", "imager_grid", "imager_degrid", "imager_plan_destroy",
-           "imager_grid_image_transform", "imager_debug_index", "imager_debug_kernels", "imager_plan_info",
+           "imager_grid_image_transform", "imager_mosaic_correct", "imager_debug_index", "imager_debug_kernels", "imager_plan_info",
            "imager_last_launch_count", "imager_last_error")
 
 
@@ -57,6 +57,7 @@ def load_library() -> ctypes.CDLL:
     lib.imager_degrid.argtypes = [c_void_p, c_int64, c_void_p, c_void_p, c_void_p, c_void_p, c_uint32, c_void_p]
     lib.imager_plan_destroy.argtypes = [c_void_p]
     lib.imager_grid_image_transform.argtypes = [c_void_p, c_void_p, c_int32, c_double, c_void_p]
+    lib.imager_mosaic_correct.argtypes = [c_void_p, c_void_p, c_void_p]
     lib.imager_debug_index.argtypes = [c_void_p, c_int64, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p,
                                        POINTER(c_int64), c_void_p]
     lib.imager_debug_kernels.argtypes = [c_void_p, c_int32, c_int32, c_void_p, POINTER(c_int32)]
@@ -171,6 +172,12 @@ class Plan:
         import torch
         _check(load_library().imager_grid_image_transform(self._h, _dev_ptr(data, torch.complex64, "data"), direction,
                                                           float(norm), _stream_ptr(stream)), "imager_grid_image_transform")
+
+    def mosaic_correct(self, image, stream=None):
+        """Eq. 1: multiply the image planes by gamma(l, m) in place (MOSAIC_PB plans)."""
+        import torch
+        _check(load_library().imager_mosaic_correct(self._h, _dev_ptr(image, torch.complex64, "image"), _stream_ptr(stream)),
+               "imager_mosaic_correct")
 
     def last_launch_count(self) -> int:
         return int(load_library().imager_last_launch_count(self._h))

@@ -96,6 +96,7 @@ extern "C" int imager_plan_create(const imager_params* params, void* cuda_stream
     imager_plan* pl = new (std::nothrow) imager_plan();
     if (!pl) return IMAGER_ERR_NOMEM;
     pl->p = *params;
+    if (params->pointing_lm) pl->pointing_lm.assign(params->pointing_lm, params->pointing_lm + 2 * (size_t)params->n_aplanes);
     pl->p.pa_rad = nullptr;
     pl->p.pointing_lm = nullptr;
     pl->p.user_tables = pl->p.user_tables_degrid = nullptr;
@@ -211,6 +212,16 @@ extern "C" int imager_grid_image_transform(imager_plan* plan, float* data, int32
     g_err[0] = 0;
     if (!plan || !data) { set_error("NULL argument"); return IMAGER_ERR_INVALID_ARG; }
     return grid_image_transform(plan, (float2*)data, direction, norm, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int imager_mosaic_correct(imager_plan* plan, float* image, void* cuda_stream) {
+    g_err[0] = 0;
+    if (!plan || !image) { set_error("NULL argument"); return IMAGER_ERR_INVALID_ARG; }
+    if (plan->p.kernel_mode != IMAGER_MODE_MOSAIC_PB) {
+        set_error("imager_mosaic_correct needs a MOSAIC_PB plan");
+        return IMAGER_ERR_INVALID_ARG;
+    }
+    return mosaic_correct(plan, (float2*)image, (cudaStream_t)cuda_stream);
 }
 
 extern "C" int imager_debug_index(imager_plan* plan, int64_t nvis, const float* uvw, const int32_t* a_index,

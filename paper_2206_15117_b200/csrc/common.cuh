@@ -60,6 +60,8 @@ struct imager_plan {
     int64_t max_items = 0;
 
     double* d_taper = nullptr;           // [N] psi(2(x-N/2)/N) for imager_grid_image_transform
+    std::vector<double> pointing_lm;     // [n_aplanes][2] copy of the caller's pointing offsets (MOSAIC_PB)
+    float* d_gamma = nullptr;            // [N][N] Eq. 1 weighting correction, built by the first imager_mosaic_correct
     void* fft_plan = nullptr;            // cufftHandle stored as intptr
     bool fft_ready = false;
 
@@ -100,5 +102,6 @@ int build_tables(imager_plan* pl, const imager_params* user, cudaStream_t st);
 // transform.cu
 int grid_image_transform(imager_plan* pl, float2* data, int direction, double norm, cudaStream_t st);
 void destroy_transform(imager_plan* pl);
+int mosaic_correct(imager_plan* pl, float2* image, cudaStream_t st);
 
 }  // namespace imager

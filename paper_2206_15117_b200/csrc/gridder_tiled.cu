@@ -50,7 +50,7 @@ constexpr int kStageSlots = 40;                       // gridding: 32 descriptor
 constexpr int kGridStageBytes = (kGridThreads / 32) * kStageSlots * 16;
 constexpr int kMaxSmem = 227 * 1024;
 constexpr int kTableBudget = kMaxSmem - kStageBytes - 32 * 1024 - 1024;   // stage + degridding reduction buffer + static
-constexpr int64_t kMaxPlanCells = 48 << 20;           // (geometry unit, strip) pairs the planner may enumerate
+constexpr int64_t kMaxPlanCells = (int64_t)1 << 30;   // (geometry unit, strip) pairs: 12 bytes of planner state each
 constexpr uint32_t kTapBias = 1u << 20;
 
 struct SetPlan {           // per kernel set (host-built)

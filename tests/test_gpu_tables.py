@@ -105,3 +105,30 @@ def test_end_to_end_with_library_tables_close_to_oracle():
         plan.grid(torch.from_numpy(uvw).cuda(), torch.from_numpy(vis).cuda(), torch.from_numpy(wts).cuda(), grid)
         g = grid.cpu().numpy()
     assert np.abs(g - out["grid"]).max() < 1e-5 * np.abs(out["grid"]).max()
+
+
+def test_mosaic_weighting_correction_eq1():
+    """imager_mosaic_correct multiplies the image by gamma(l, m) of Eq. 1; the oracle builds gamma from
+    its own Airy power beams at the same pixel coordinates."""
+    import torch
+    from paper_2206_15117_b200 import Plan, ImagerError
+    params = TABLE_CASES["mosaic"]
+    n, cell = params["grid_size"], params["cell_size_rad"]
+    ax = (np.arange(n) - n // 2) * cell
+    ll, mm = np.meshgrid(ax, ax)                                     # x (l) along the last axis
+    beams = np.stack([ok.airy(np.hypot(ll - la, mm - ma), params["dish_diameter_m"], params["freq_hz"]) ** 2
+                      for la, ma in params["pointing_lm"]])
+    gamma = oi.mosaic_gamma(beams)
+    rng = np.random.default_rng(5)
+    img = (rng.standard_normal((1, n, n)) + 1j * rng.standard_normal((1, n, n))).astype(np.complex64)
+    with Plan(params, 16) as plan:
+        d = torch.from_numpy(img).cuda()
+        plan.mosaic_correct(d)
+        plan.mosaic_correct(d)                                       # second call uses the cached gamma
+        torch.cuda.synchronize()
+        got = d.cpu().numpy()
+    ref = img.astype(np.complex128) * gamma ** 2
+    assert np.max(np.abs(got - ref) / np.abs(ref)) < 5e-6           # float32 gamma and two float32 products
+    with Plan(TABLE_CASES["pswf"], 16) as plan:
+        with pytest.raises(ImagerError):
+            plan.mosaic_correct(torch.zeros((1, 128, 128), dtype=torch.complex64, device="cuda"))
