@@ -296,36 +296,57 @@ __global__ void __launch_bounds__(256) sort_items_kernel(int n_items, const Item
         if (k * 32 + lane < n_hits) hit_rec[out + atomicAdd(&s_bin[warp][ctrl_variant(r[k].y >> 24)], 1)] = r[k];
 }
 
-// one thread block per geometry unit: blocks of about kBlockHits hits (whole items), replicated for every Mueller
-// element sc = s * n_corr + c.  Block order is irrelevant (a work queue consumes them).
+// one thread block per geometry unit: blocks of whole items, replicated for every Mueller element sc = s * n_corr + c.
+// All but the last 1/kTailFrac of a unit's blocks go to the FRONT of `blocks` (about kBlockHits hits each), the rest into
+// blocks of kBlockHits / kTailDiv hits at its BACK; the work queue serves the front part first, so that the kernel
+// ends on small blocks (a short tail) without paying their overhead throughout.
+#ifndef IMAGER_TAIL_DIV
+#define IMAGER_TAIL_DIV 4
+#endif
+#ifndef IMAGER_TAIL_FRAC
+#define IMAGER_TAIL_FRAC 16
+#endif
+constexpr int kTailDiv = IMAGER_TAIL_DIV, kTailFrac = IMAGER_TAIL_FRAC;
+__device__ __forceinline__ int first_item_at(const Item* __restrict__ item_rec, int lo, int hi, int64_t limit) {
+    while (lo < hi) {                                     // first item whose hit_begin >= limit
+        const int mid = (lo + hi) >> 1;
+        if (item_rec[mid].hit_begin < limit) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+
 __global__ void plan_blocks_kernel(const Geometry g, const int32_t* __restrict__ hit_start, const int32_t* __restrict__ item_start,
-                                   const Item* __restrict__ item_rec, Block* __restrict__ blocks, int32_t* __restrict__ n_blocks,
-                                   int max_blocks) {
-    __shared__ int s_base;
+                                   const Item* __restrict__ item_rec, Block* __restrict__ blocks, int32_t* __restrict__ n_front,
+                                   int32_t* __restrict__ n_back, int cap_blocks) {
+    __shared__ int s_front, s_back;
     const int gu = blockIdx.x;
     const int n_sc = g.n_pol * g.n_corr;
     const int64_t c0 = (int64_t)gu * g.n_strips, c1 = c0 + g.n_strips;
     const int h0 = hit_start[c0], h1 = hit_start[c1], i0 = item_start[c0], i1 = item_start[c1];
     if (h1 == h0) return;
-    const int nb = (h1 - h0 + kBlockHits - 1) / kBlockHits;
-    if (threadIdx.x == 0) s_base = atomicAdd(n_blocks, nb * n_sc);
+    const int nb_all = (h1 - h0 + kBlockHits - 1) / kBlockHits;
+    const int nb_front = nb_all - (nb_all + kTailFrac - 1) / kTailFrac;   // whole big blocks in the front part
+    const int64_t hs = (int64_t)h0 + (int64_t)nb_front * kBlockHits;  // the tail part starts here
+    constexpr int kSmall = kBlockHits / kTailDiv;
+    const int nb_back = (int)((h1 - hs + kSmall - 1) / kSmall);
+    if (threadIdx.x == 0) {
+        s_front = atomicAdd(n_front, nb_front * n_sc);
+        s_back = atomicAdd(n_back, nb_back * n_sc);
+    }
     __syncthreads();
-    const int base = s_base;
-    if (base + nb * n_sc > max_blocks) return;                        // cannot happen: max_blocks is an upper bound
-    for (int b = threadIdx.x; b < nb; b += blockDim.x) {
-        int bounds[2];                                                // items [first, last): hit_begin in [h0 + b K, h0 + (b + 1) K)
-#pragma unroll
-        for (int e = 0; e < 2; ++e) {
-            const int64_t limit = (int64_t)h0 + (int64_t)(b + e) * kBlockHits;
-            int lo = i0, hi = i1;
-            while (lo < hi) {
-                const int mid = (lo + hi) >> 1;
-                if (item_rec[mid].hit_begin < limit) lo = mid + 1; else hi = mid;
-            }
-            bounds[e] = lo;
+    const int is = first_item_at(item_rec, i0, i1, hs);               // first item of the tail part
+    for (int b = threadIdx.x; b < nb_front + nb_back; b += blockDim.x) {
+        const bool front = b < nb_front;
+        const int k = front ? b : b - nb_front, nbk = front ? nb_front : nb_back;
+        const int64_t lo_hit = front ? (int64_t)h0 + (int64_t)k * kBlockHits : hs + (int64_t)k * kSmall;
+        const int64_t hi_hit = front ? lo_hit + kBlockHits : lo_hit + kSmall;
+        const int first = (k == 0) ? (front ? i0 : is) : first_item_at(item_rec, i0, i1, lo_hit);
+        const int last = (k == nbk - 1) ? (front ? is : i1) : first_item_at(item_rec, i0, i1, hi_hit);
+        const int cnt = max(last - first, 0);                         // items are whole: a small block may come out empty
+        for (int sc = 0; sc < n_sc; ++sc) {
+            const int slot = front ? s_front + sc * nb_front + k : cap_blocks - 1 - (s_back + sc * nb_back + k);
+            blocks[slot] = Block{gu, sc, first, cnt};
         }
-        if (b == nb - 1) bounds[1] = i1;
-        for (int sc = 0; sc < n_sc; ++sc) blocks[base + sc * nb + b] = Block{gu, sc, bounds[0], bounds[1] - bounds[0]};
     }
 }
 
@@ -335,7 +356,9 @@ struct TiledArgs {
     const uint2* hit_rec;
     const Item* items;
     const Block* blocks;
-    const int32_t* n_blocks;
+    const int32_t* n_front;     // blocks at the front of `blocks` (served first)
+    const int32_t* n_back;      // blocks at its back: entry cap_blocks - 1 - k
+    int32_t cap_blocks;
     int32_t* queue;
     const float2* tab;
     const int64_t* set_offset;
@@ -479,7 +502,7 @@ grid_tiled_kernel(const TiledArgs a, const float2* __restrict__ sval, float2* __
     __shared__ int s_block, s_next;
     const int lane = threadIdx.x & 31, lx = lane & (kLaneW - 1), ly = lane >> 3;
     const Geometry g = a.g;
-    const int n_blocks = *a.n_blocks;
+    const int n_front = *a.n_front, n_blocks = n_front + *a.n_back;
     int cur_gu = -1, cur_sc = -1;
     for (;;) {
         __syncthreads();                                   // everyone is done with the previous block
@@ -489,7 +512,8 @@ grid_tiled_kernel(const TiledArgs a, const float2* __restrict__ sval, float2* __
         }
         __syncthreads();
         if (s_block >= n_blocks) break;
-        const Block blk = a.blocks[s_block];
+        const Block blk = a.blocks[s_block < n_front ? s_block : a.cap_blocks - 1 - (s_block - n_front)];
+        if (blk.item_count == 0) continue;
         const int kset = a.gu_set[blk.gu];
         const SetPlan sp = a.set_plan[kset];
         const int S = a.set_support[kset];
@@ -641,7 +665,7 @@ degrid_tiled_kernel(const TiledArgs a, const float2* __restrict__ grid, float2* 
     __shared__ int s_block, s_next;
     const int lane = threadIdx.x & 31, lx = lane & (kLaneW - 1), ly = lane >> 3;
     const Geometry g = a.g;
-    const int n_blocks = *a.n_blocks;
+    const int n_front = *a.n_front, n_blocks = n_front + *a.n_back;
     int cur_gu = -1, cur_sc = -1;
     for (;;) {
         __syncthreads();
@@ -651,7 +675,8 @@ degrid_tiled_kernel(const TiledArgs a, const float2* __restrict__ grid, float2* 
         }
         __syncthreads();
         if (s_block >= n_blocks) break;
-        const Block blk = a.blocks[s_block];
+        const Block blk = a.blocks[s_block < n_front ? s_block : a.cap_blocks - 1 - (s_block - n_front)];
+        if (blk.item_count == 0) continue;
         const int kset = a.gu_set[blk.gu];
         const SetPlan sp = a.set_plan[kset];
         const int S = a.set_support[kset];
@@ -753,6 +778,7 @@ struct TiledState {
     uint2* d_sgeo = nullptr;
     float2* d_sval = nullptr;
     int64_t plan_epoch = -1;
+    int32_t blocks_cap = 0;               // the two-ended block queue lives in d_blocks[0 .. blocks_cap)
     Geometry g;
     int smem_bytes = 0;
 };
@@ -898,7 +924,12 @@ static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
         return IMAGER_ERR_UNSUPPORTED;
     }
     const int n_sc = g.n_pol * g.n_corr;
-    const int64_t max_blocks = ((int64_t)g.n_gu + n_hits / kBlockHits + 1) * n_sc;
+    const int64_t max_blocks = (n_hits / kBlockHits + n_hits / (kTailFrac * (kBlockHits / kTailDiv)) + (int64_t)g.n_gu * (2 * kTailDiv + 4) + 4) * n_sc;
+    if (max_blocks > 0x7fffffff) {
+        set_error("too many work blocks");
+        return IMAGER_ERR_UNSUPPORTED;
+    }
+    st->blocks_cap = (int32_t)max_blocks;
     rc = grow(&st->d_hit_rec, &st->cap_hits, n_hits + 1);
     if (rc) return rc;
     rc = grow(&st->d_item_rec, &st->cap_items, n_items + 1);
@@ -915,8 +946,9 @@ static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
                                                                              st->d_hit_rec);
     pl->last_launches += 2;
     IMAGER_CUDA(cudaMemsetAsync(pl->d_counters + 9, 0, sizeof(int32_t), stream));
+    IMAGER_CUDA(cudaMemsetAsync(pl->d_counters + 12, 0, sizeof(int32_t), stream));
     plan_blocks_kernel<<<g.n_gu, 128, 0, stream>>>(g, st->d_hits, st->d_items, st->d_item_rec, st->d_blocks, pl->d_counters + 9,
-                                                   (int)std::min<int64_t>(st->cap_blocks, 0x7fffffff));
+                                                   pl->d_counters + 12, st->blocks_cap);
     pl->last_launches += 2;
     IMAGER_CUDA(cudaGetLastError());
     st->plan_epoch = pl->index_epoch;
@@ -928,7 +960,9 @@ static void fill_args(imager_plan* pl, TiledState* st, TiledArgs& a, const float
     a.hit_rec = st->d_hit_rec;
     a.items = st->d_item_rec;
     a.blocks = st->d_blocks;
-    a.n_blocks = pl->d_counters + 9;
+    a.n_front = pl->d_counters + 9;
+    a.n_back = pl->d_counters + 12;
+    a.cap_blocks = st->blocks_cap;
     a.queue = pl->d_counters + 8;
     a.tab = tab;
     a.set_offset = pl->d_set_offset;
