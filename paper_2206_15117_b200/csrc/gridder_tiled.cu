@@ -38,10 +38,10 @@ constexpr int kGridThreads = IMAGER_GRID_THREADS;     // gridding kernel: thread
 #define IMAGER_CHUNK3 4
 #endif
 #ifndef IMAGER_ITEM_HITS
-#define IMAGER_ITEM_HITS 256
+#define IMAGER_ITEM_HITS 384
 #endif
 #ifndef IMAGER_BLOCK_HITS
-#define IMAGER_BLOCK_HITS 32768
+#define IMAGER_BLOCK_HITS 73728
 #endif
 constexpr int kItemHits = IMAGER_ITEM_HITS;                        // hits per work item (one flush / strip load each)
 constexpr int kBlockHits = IMAGER_BLOCK_HITS;                     // hits per CTA-level block
