@@ -29,7 +29,10 @@ constexpr int kLaneW = 8, kLaneH = 4;                 // lane block
 constexpr int kNX = 2, kNY = 8;                       // replications: strip = 16 x 32 cells
 constexpr int kStripW = kLaneW * kNX, kStripH = kLaneH * kNY;
 constexpr int kPadY = kLaneH - 1, kPadX = kLaneW - 1;
-constexpr int kTiledThreads = 512, kWarps = kTiledThreads / 32;
+#ifndef IMAGER_DEGRID_THREADS
+#define IMAGER_DEGRID_THREADS 512
+#endif
+constexpr int kTiledThreads = IMAGER_DEGRID_THREADS, kWarps = kTiledThreads / 32;   // degridding kernel
 #ifndef IMAGER_GRID_THREADS
 #define IMAGER_GRID_THREADS 768
 #endif
@@ -49,7 +52,10 @@ constexpr int kStageBytes = kWarps * 32 * 16;         // per-warp hit descriptor
 constexpr int kStageSlots = 40;                       // gridding: 32 descriptors + the one read past a batch's end
 constexpr int kGridStageBytes = (kGridThreads / 32) * kStageSlots * 16;
 constexpr int kMaxSmem = 227 * 1024;
-constexpr int kTableBudget = kMaxSmem - kStageBytes - 32 * 1024 - 1024;   // stage + degridding reduction buffer + static
+constexpr int kRedSlots = 8;                           // degridding: hits per transposed reduction
+constexpr int kRedBytes = kWarps * kRedSlots * 32 * 8;
+constexpr int kTableBudget = kMaxSmem - kStageBytes - kRedBytes - 1024;   // stage + degridding reduction buffer + static
+static_assert(kGridStageBytes <= kStageBytes + kRedBytes, "the gridding kernel's staging must fit beside the tables");
 constexpr int64_t kMaxPlanCells = (int64_t)1 << 30;   // (geometry unit, strip) pairs: 12 bytes of planner state each
 constexpr uint32_t kTapBias = 1u << 20;
 
@@ -595,8 +601,6 @@ grid_tiled_kernel(const TiledArgs a, const float2* __restrict__ sval, float2* __
 // The 32 partial sums of a hit go to a per-warp shared buffer red[slot][lane]; every 8 hits the buffer is summed
 // by a transposed read (lane = slot + 8 * quarter sums 8 columns, two shuffles join the quarters) and the result is
 // added to the visibility's sorted-order sum with one red.global.add.v2.f32 per hit.
-constexpr int kRedSlots = 8;
-constexpr int kRedBytes = kWarps * kRedSlots * 32 * 8;      // 32 KB
 
 __device__ __forceinline__ void sts64(uint32_t addr, float2 v) {
     asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(v.x), "f"(v.y) : "memory");
