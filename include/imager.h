@@ -102,6 +102,12 @@ typedef struct imager_record {
  * Errors: INVALID_ARG (bad sizes, NULL), UNSUPPORTED (mode / shape combination not built), NOMEM, CUDA. */
 int imager_plan_create(const imager_params* params, void* cuda_stream, imager_plan** out_plan);
 
+/* Steps A1 + A2 on their own: index and bucket (uvw, a_index) and plan the work lists of the gridding / degridding
+ * kernels, so that later imager_grid / imager_degrid calls with IMAGER_REUSE_INDEX start at once (e.g. while the
+ * visibilities are still being copied to the device).  uvw dev float32 [nvis][3], a_index dev int32 [nvis] or NULL.
+ * Synchronises the stream once (the list sizes are read back).  Errors: INVALID_ARG, TOO_MANY_VIS, NOMEM, CUDA. */
+int imager_index(imager_plan* plan, int64_t nvis, const float* uvw, const int32_t* a_index, void* cuda_stream);
+
 /* Gridding.  Accumulates into `grid` (the caller zeroes it); visibilities whose footprint leaves the
  * grid are skipped and counted (R8).  uvw dev float32 [nvis][3] in wavelengths ("baseline vectors ... in
  * units of wavelength"); vis dev complex64 [nvis][n_corr]; weights dev float32 [nvis][n_corr]; a_index dev

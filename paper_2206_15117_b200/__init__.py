@@ -11,6 +11,10 @@ def imager_plan_create(params: dict, max_nvis: int, user_tables=None, user_table
     return Plan(params, max_nvis, user_tables, user_tables_degrid, stream)
 
 
+def imager_index(plan: Plan, uvw, a_index=None, stream=None):
+    plan.index(uvw, a_index, stream)
+
+
 def imager_grid(plan: Plan, uvw, vis, weights, grid, a_index=None, sum_weights=None, flags: int = 0, stream=None):
     plan.grid(uvw, vis, weights, grid, a_index, sum_weights, flags, stream)
 

@@ -21,7 +21,7 @@ PATH_REFERENCE = 2
 PATH_SMEM = 4
 PATH_TMEM = 8
 
-EXPORTS = ("imager_plan_create", "imager_grid", "imager_degrid", "imager_plan_destroy",
+EXPORTS = ("imager_plan_create", "imager_index", "imager_grid", "imager_degrid", "imager_plan_destroy",
            "imager_grid_image_transform", "imager_mosaic_correct", "imager_debug_index", "imager_debug_kernels", "imager_plan_info",
            "imager_last_launch_count", "imager_last_error")
 
@@ -54,6 +54,7 @@ def load_library() -> ctypes.CDLL:
     lib.imager_plan_create.argtypes = [POINTER(ImagerParams), c_void_p, POINTER(c_void_p)]
     lib.imager_grid.argtypes = [c_void_p, c_int64, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_uint32,
                                 c_void_p]
+    lib.imager_index.argtypes = [c_void_p, c_int64, c_void_p, c_void_p, c_void_p]
     lib.imager_degrid.argtypes = [c_void_p, c_int64, c_void_p, c_void_p, c_void_p, c_void_p, c_uint32, c_void_p]
     lib.imager_plan_destroy.argtypes = [c_void_p]
     lib.imager_grid_image_transform.argtypes = [c_void_p, c_void_p, c_int32, c_double, c_void_p]
@@ -148,6 +149,13 @@ class Plan:
         self.close()
 
     # ---- hot path -------------------------------------------------------------------------------------------
+    def index(self, uvw, a_index=None, stream=None):
+        """A1 + A2 ahead of time; follow with grid / degrid calls that pass REUSE_INDEX."""
+        import torch
+        nvis = int(uvw.shape[0])
+        _check(load_library().imager_index(self._h, nvis, _dev_ptr(uvw, torch.float32, "uvw"),
+                                           _dev_ptr(a_index, torch.int32, "a_index"), _stream_ptr(stream)), "imager_index")
+
     def grid(self, uvw, vis, weights, grid, a_index=None, sum_weights=None, flags: int = 0, stream=None):
         """imager_grid: accumulates into `grid` (complex64 [n_pol,N,N] CUDA tensor)."""
         import torch

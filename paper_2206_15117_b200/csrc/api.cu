@@ -177,6 +177,16 @@ static int ensure_index(imager_plan* pl, int64_t nvis, const float* uvw, const i
     return run_index_and_sort(pl, nvis, uvw, a_index, st);
 }
 
+extern "C" int imager_index(imager_plan* plan, int64_t nvis, const float* uvw, const int32_t* a_index, void* cuda_stream) {
+    g_err[0] = 0;
+    if (!plan) { set_error("plan is NULL"); return IMAGER_ERR_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    plan->last_launches = 0;
+    int rc = ensure_index(plan, nvis, uvw, a_index, 0, st);
+    if (rc) return rc;
+    return tiled_supported(plan) ? tiled_prepare(plan, nvis, st) : 0;
+}
+
 extern "C" int imager_grid(imager_plan* plan, int64_t nvis, const float* uvw, const float* vis, const float* weights,
                            const int32_t* a_index, float* grid, double* sum_weights, uint32_t flags, void* cuda_stream) {
     g_err[0] = 0;

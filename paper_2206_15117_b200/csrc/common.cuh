@@ -89,6 +89,7 @@ int launch_grid_tiled(imager_plan* pl, int64_t nvis, const float2* vis, const fl
                       cudaStream_t st);
 int launch_degrid_tiled(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, cudaStream_t st);
 void tiled_release(imager_plan* pl);
+int tiled_prepare(imager_plan* pl, int64_t nvis, cudaStream_t st);
 
 // gridder_tmem.cu
 bool tmem_supported(const imager_plan* pl);

@@ -975,6 +975,12 @@ static void fill_args(imager_plan* pl, TiledState* st, TiledArgs& a, const float
     a.gu_set = st->d_gu_set;
 }
 
+// hit lists for the current index (imager_index: planning ahead of the first gridding / degridding call)
+int tiled_prepare(imager_plan* pl, int64_t nvis, cudaStream_t stream) {
+    if (nvis == 0) return 0;
+    return prepare(pl, state_of(pl), stream);
+}
+
 int launch_grid_tiled(imager_plan* pl, int64_t nvis, const float2* vis, const float* weights, float2* grid,
                       cudaStream_t stream) {
     if (nvis == 0) return 0;

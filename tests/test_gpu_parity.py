@@ -193,3 +193,29 @@ def test_adjointness_on_gpu(torch_cuda):
             lhs = torch.vdot(g.to(torch.complex128).flatten(), gv.to(torch.complex128).flatten()).item()
             rhs = torch.vdot(hg.to(torch.complex128).flatten(), d_vis.to(torch.complex128).flatten()).item()
             assert abs(lhs - rhs) <= 1e-6 * abs(lhs), (case, lhs, rhs)
+
+
+def test_index_ahead_of_grid(torch_cuda, oracle_lib):
+    """imager_index (A1 + A2 on their own) followed by REUSE_INDEX calls gives what the one-call path gives."""
+    torch = torch_cuda
+    from paper_2206_15117_b200 import Plan, REUSE_INDEX
+    params = CASES["wproj"]()
+    nvis = 5000
+    uvw, vis, wts, a = random_vis(params, nvis, seed=7, frac=0.45)
+    _, _, flat, offs = oracle_tables(params)
+    rec = oidx.index_visibilities(uvw, a, params)
+    ref = og.grid(rec, vis, wts, flat, offs, params)
+    n = params["grid_size"]
+    with Plan(params, nvis, user_tables=flat) as plan:
+        d_uvw, d_vis, d_wts, _ = _to_dev(torch, uvw, vis, wts, None)
+        plan.index(d_uvw)
+        assert plan.last_launch_count() > 0
+        grid = torch.zeros((1, n, n), dtype=torch.complex64, device="cuda")
+        plan.grid(d_uvw, d_vis, d_wts, grid, flags=REUSE_INDEX)
+        out = torch.empty((nvis, 1), dtype=torch.complex64, device="cuda")
+        plan.degrid(d_uvw, grid, out, flags=REUSE_INDEX)
+        torch.cuda.synchronize()
+        g = grid.cpu().numpy()
+        assert grid_error(g, ref) <= TOL
+        refd = og.degrid(rec, g, flat, offs, params)
+        assert vis_error(out.cpu().numpy(), refd, rec["drop"]) <= TOL
