@@ -57,8 +57,11 @@ enum {
                                        (same results up to summation order; for tests and A/B timing)             */
     IMAGER_PATH_SMEM = 4u,          /* use the shared-memory-tap tiled kernels (the default path; kept so that
                                        callers can name it explicitly)                                            */
-    IMAGER_PATH_TMEM = 8u           /* gridding with the taps in tensor memory (experimental, slower than the
+    IMAGER_PATH_TMEM = 8u,          /* gridding with the taps in tensor memory (experimental, slower than the
                                        default on sparse uv coverage; shapes that do not fit fall back; A/B timing) */
+    IMAGER_DEGRID_RESIDUAL = 16u    /* imager_degrid: vis_out holds the observed visibilities on entry and the
+                                       residuals V - V_model on return (the major-cycle update), fused into
+                                       the kernel's epilogue; dropped visibilities are left as they are           */
 };
 
 typedef struct imager_plan imager_plan;   /* opaque, owned by the library */
@@ -118,7 +121,8 @@ int imager_grid(imager_plan* plan, int64_t nvis, const float* uvw, const float* 
                 const int32_t* a_index, float* grid, double* sum_weights, uint32_t flags, void* cuda_stream);
 
 /* Degridding: predicts vis_out dev complex64 [nvis][n_corr] (overwritten, input order) from grid dev
- * complex64 [n_pol][N][N]; dropped visibilities predict 0.  Weights play no part. */
+ * complex64 [n_pol][N][N]; dropped visibilities predict 0.  Weights play no part.  With IMAGER_DEGRID_RESIDUAL the
+ * prediction is subtracted from what vis_out holds instead (vis_out := vis_out - V_model). */
 int imager_degrid(imager_plan* plan, int64_t nvis, const float* uvw, const int32_t* a_index, const float* grid,
                   float* vis_out, uint32_t flags, void* cuda_stream);
 

@@ -20,6 +20,7 @@ REUSE_INDEX = 1
 PATH_REFERENCE = 2
 PATH_SMEM = 4
 PATH_TMEM = 8
+DEGRID_RESIDUAL = 16
 
 EXPORTS = ("imager_plan_create", "imager_index", "imager_grid", "imager_degrid", "imager_plan_destroy",
            "imager_grid_image_transform", "imager_mosaic_correct", "imager_debug_index", "imager_debug_kernels", "imager_plan_info",

@@ -212,9 +212,10 @@ extern "C" int imager_degrid(imager_plan* plan, int64_t nvis, const float* uvw, 
     plan->last_launches = 0;
     int rc = ensure_index(plan, nvis, uvw, a_index, flags, st);
     if (rc) return rc;
+    const int residual = (flags & IMAGER_DEGRID_RESIDUAL) ? 1 : 0;
     if (!(flags & IMAGER_PATH_REFERENCE) && tiled_supported(plan))
-        return launch_degrid_tiled(plan, nvis, (const float2*)grid, (float2*)vis_out, st);
-    return launch_degrid_reference(plan, nvis, (const float2*)grid, (float2*)vis_out, nullptr, st);
+        return launch_degrid_tiled(plan, nvis, (const float2*)grid, (float2*)vis_out, residual, st);
+    return launch_degrid_reference(plan, nvis, (const float2*)grid, (float2*)vis_out, nullptr, residual, st);
 }
 
 extern "C" int imager_grid_image_transform(imager_plan* plan, float* data, int32_t direction, double norm,

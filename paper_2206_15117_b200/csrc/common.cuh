@@ -80,14 +80,14 @@ int exclusive_scan_i32(imager_plan* pl, int32_t* data, int64_t n, int32_t* tmp, 
 int launch_grid_reference(imager_plan* pl, int64_t nvis, const float2* vis, const float* weights, float2* grid,
                           const int32_t* set_mask, cudaStream_t st);
 int launch_degrid_reference(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, const int32_t* set_mask,
-                            cudaStream_t st);
+                            int residual, cudaStream_t st);
 int launch_sum_weights(imager_plan* pl, int64_t nvis, const float* weights, double* sum_weights, cudaStream_t st);
 
 // gridder_tiled.cu
 bool tiled_supported(const imager_plan* pl);
 int launch_grid_tiled(imager_plan* pl, int64_t nvis, const float2* vis, const float* weights, float2* grid,
                       cudaStream_t st);
-int launch_degrid_tiled(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, cudaStream_t st);
+int launch_degrid_tiled(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, int residual, cudaStream_t st);
 void tiled_release(imager_plan* pl);
 int tiled_prepare(imager_plan* pl, int64_t nvis, cudaStream_t st);
 

@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(256)
 degrid_ref_kernel(int64_t nvis, const imager_record* __restrict__ rec, const int32_t* __restrict__ perm,
                   const float2* __restrict__ grid, const float2* __restrict__ tab,
                   const int64_t* __restrict__ set_offset, const int32_t* __restrict__ set_support,
-                  const int32_t* __restrict__ set_mask, int N, int O, float2* __restrict__ vis_out) {
+                  const int32_t* __restrict__ set_mask, int N, int O, int residual, float2* __restrict__ vis_out) {
     const int lane = threadIdx.x & 31;
     const int64_t warp0 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int64_t n_warps = ((int64_t)gridDim.x * blockDim.x) >> 5;
@@ -104,7 +104,10 @@ degrid_ref_kernel(int64_t nvis, const imager_record* __restrict__ rec, const int
         }
         if (lane == 0) {
 #pragma unroll
-            for (int c = 0; c < NC; ++c) vis_out[(int64_t)k * NC + c] = acc[c];
+            for (int c = 0; c < NC; ++c) {
+                float2* o = vis_out + (int64_t)k * NC + c;
+                *o = residual ? make_float2(o->x - acc[c].x, o->y - acc[c].y) : acc[c];
+            }
         }
     }
 }
@@ -155,16 +158,16 @@ int launch_grid_reference(imager_plan* pl, int64_t nvis, const float2* vis, cons
 }
 
 int launch_degrid_reference(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, const int32_t* set_mask,
-                            cudaStream_t st) {
+                            int residual, cudaStream_t st) {
     if (nvis == 0) return 0;
     const unsigned blocks = (unsigned)std::min<int64_t>((nvis + 7) / 8, 16 * kNumSMs);
     const int N = pl->p.grid_size, O = pl->p.oversample;
     if (pl->p.n_corr == 1)
         degrid_ref_kernel<1, 1><<<blocks, 256, 0, st>>>(nvis, pl->d_rec, pl->d_perm[pl->sorted_buf], grid, pl->d_tab_degrid,
-                                                        pl->d_set_offset, pl->d_set_support, set_mask, N, O, vis_out);
+                                                        pl->d_set_offset, pl->d_set_support, set_mask, N, O, residual, vis_out);
     else
         degrid_ref_kernel<4, 4><<<blocks, 256, 0, st>>>(nvis, pl->d_rec, pl->d_perm[pl->sorted_buf], grid, pl->d_tab_degrid,
-                                                        pl->d_set_offset, pl->d_set_support, set_mask, N, O, vis_out);
+                                                        pl->d_set_offset, pl->d_set_support, set_mask, N, O, residual, vis_out);
     pl->last_launches++;
     IMAGER_CUDA(cudaGetLastError());
     return 0;

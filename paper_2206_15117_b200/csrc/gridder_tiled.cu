@@ -119,15 +119,20 @@ __global__ void gather_values_kernel(const int32_t* __restrict__ counters, const
     }
 }
 
-// degridding epilogue: sorted-order sums -> vis_out in input order (dropped visibilities predict 0)
+// degridding epilogue: sorted-order sums -> vis_out in input order (dropped visibilities predict 0); with `residual`
+// the prediction is subtracted from what vis_out holds (V - V_model, the major-cycle update)
 template <int NC>
 __global__ void scatter_values_kernel(int64_t nvis, const int32_t* __restrict__ counters, const int32_t* __restrict__ perm,
-                                      const float2* __restrict__ sval, float2* __restrict__ vis_out) {
+                                      const float2* __restrict__ sval, int residual, float2* __restrict__ vis_out) {
     const int n_kept = counters[0];
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvis; i += (int64_t)gridDim.x * blockDim.x) {
         const int64_t k = perm[i];
 #pragma unroll
-        for (int c = 0; c < NC; ++c) vis_out[k * NC + c] = i < n_kept ? sval[i * NC + c] : make_float2(0.f, 0.f);
+        for (int c = 0; c < NC; ++c) {
+            const float2 m = i < n_kept ? sval[i * NC + c] : make_float2(0.f, 0.f);
+            float2* o = vis_out + k * NC + c;
+            *o = residual ? make_float2(o->x - m.x, o->y - m.y) : m;
+        }
     }
 }
 
@@ -1004,7 +1009,7 @@ int launch_grid_tiled(imager_plan* pl, int64_t nvis, const float2* vis, const fl
     return 0;
 }
 
-int launch_degrid_tiled(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, cudaStream_t stream) {
+int launch_degrid_tiled(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, int residual, cudaStream_t stream) {
     if (nvis == 0) return 0;
     TiledState* st = state_of(pl);
     int rc = prepare(pl, st, stream);
@@ -1018,10 +1023,10 @@ int launch_degrid_tiled(imager_plan* pl, int64_t nvis, const float2* grid, float
     const unsigned gb = 4 * kNumSMs;
     if (nc == 1) {
         degrid_tiled_kernel<1><<<kNumSMs, kTiledThreads, smem, stream>>>(a, grid, st->d_sval);
-        scatter_values_kernel<1><<<gb, 256, 0, stream>>>(nvis, pl->d_counters, pl->d_perm[pl->sorted_buf], st->d_sval, vis_out);
+        scatter_values_kernel<1><<<gb, 256, 0, stream>>>(nvis, pl->d_counters, pl->d_perm[pl->sorted_buf], st->d_sval, residual, vis_out);
     } else {
         degrid_tiled_kernel<4><<<kNumSMs, kTiledThreads, smem, stream>>>(a, grid, st->d_sval);
-        scatter_values_kernel<4><<<gb, 256, 0, stream>>>(nvis, pl->d_counters, pl->d_perm[pl->sorted_buf], st->d_sval, vis_out);
+        scatter_values_kernel<4><<<gb, 256, 0, stream>>>(nvis, pl->d_counters, pl->d_perm[pl->sorted_buf], st->d_sval, residual, vis_out);
     }
     pl->last_launches += 2;
     IMAGER_CUDA(cudaGetLastError());

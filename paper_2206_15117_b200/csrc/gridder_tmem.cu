@@ -862,7 +862,7 @@ int launch_grid_tmem(imager_plan* pl, int64_t nvis, const float2* vis, const flo
 }
 
 int launch_degrid_tmem(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, cudaStream_t stream) {
-    return launch_degrid_tiled(pl, nvis, grid, vis_out, stream);
+    return launch_degrid_tiled(pl, nvis, grid, vis_out, 0, stream);
 }
 
 }  // namespace imager

@@ -219,3 +219,30 @@ def test_index_ahead_of_grid(torch_cuda, oracle_lib):
         assert grid_error(g, ref) <= TOL
         refd = og.degrid(rec, g, flat, offs, params)
         assert vis_error(out.cpu().numpy(), refd, rec["drop"]) <= TOL
+
+
+@pytest.mark.parametrize("flags", [0, 2], ids=["default", "reference"])
+def test_degrid_residual_flag(torch_cuda, oracle_lib, flags):
+    """IMAGER_DEGRID_RESIDUAL: vis_out := vis_out - V_model (the major-cycle update), against the oracle's prediction."""
+    torch = torch_cuda
+    from paper_2206_15117_b200 import Plan, DEGRID_RESIDUAL
+    params = CASES["awproj"]()
+    nvis = 4000
+    uvw, vis, _, a = random_vis(params, nvis, seed=13, frac=0.5, a_planes=True)
+    _, _, flat, offs = oracle_tables(params)
+    rec = oidx.index_visibilities(uvw, a, params)
+    n, npol = params["grid_size"], params["n_pol"]
+    rng = np.random.default_rng(3)
+    g = (rng.standard_normal((npol, n, n)) + 1j * rng.standard_normal((npol, n, n))).astype(np.complex64)
+    refd = og.degrid(rec, g, flat, offs, params)
+    with Plan(params, nvis, user_tables=flat) as plan:
+        d_uvw, d_vis, _, d_a = _to_dev(torch, uvw, vis, None, a)
+        d_g = torch.from_numpy(g).cuda()
+        res = d_vis.clone()
+        plan.degrid(d_uvw, d_g, res, d_a, flags=flags | DEGRID_RESIDUAL)
+        torch.cuda.synchronize()
+        got = res.cpu().numpy()
+    want = vis.astype(np.complex128) - refd["vis"]
+    assert np.array_equal(got[rec["drop"]], vis[rec["drop"]])             # dropped: predicted 0, left as they are
+    ok = refd["norm"] > 0
+    assert float(np.max(np.abs(got[ok] - want[ok]) / (refd["norm"][ok] + np.abs(vis[ok])))) <= TOL
