@@ -16,7 +16,7 @@ __global__ void __launch_bounds__(kThreads,1) k(uint32_t mask,int bc,float* out,
   const int lane=threadIdx.x&31, warp=threadIdx.x>>5;
   const bool p=(mask>>lane)&1;
   const int esz=(W==0)?8:(W==1)?4:16;
-  const uint32_t sbase=(uint32_t)__cvta_generic_to_shared(sm)+(bc?0:lane*esz)+warp*512;
+  const uint32_t sbase=(uint32_t)__cvta_generic_to_shared(sm)+(bc==0?lane*esz:bc==2?(lane>>4)*272:bc==3?(lane>>3)*272:0)+warp*512;
   float acc=0.f;
   long long t0=clock64();
   #pragma unroll 1
@@ -40,12 +40,13 @@ int main(){
   CK(cudaFuncSetAttribute(k<1>,cudaFuncAttributeMaxDynamicSharedMemorySize,smem));
   CK(cudaFuncSetAttribute(k<2>,cudaFuncAttributeMaxDynamicSharedMemorySize,smem));
   struct {const char* n; uint32_t m;} masks[]={{"all",0xffffffffu},{"lanes0-15",0x0000ffffu},{"lanes16-31",0xffff0000u},{"even",0x55555555u},{"lanes0-7",0xffu},{"0-7,16-23",0x00ff00ffu},{"0-3 of each 8",0x0f0f0f0fu},{"lanes0-23",0x00ffffffu},{"lane0",1u}};
-  for(int w=0;w<3;++w) for(int bc=0;bc<2;++bc) for(auto& mk:masks){
+  for(int w=0;w<3;++w) for(int bc=0;bc<4;++bc) for(auto& mk:masks){
+    if(bc>=2 && mk.m!=0xffffffffu) continue;
     auto launch=[&]{ if(w==0) k<0><<<148,kThreads,smem>>>(mk.m,bc,out,cyc); else if(w==1) k<1><<<148,kThreads,smem>>>(mk.m,bc,out,cyc); else k<2><<<148,kThreads,smem>>>(mk.m,bc,out,cyc); };
     launch(); CK(cudaDeviceSynchronize()); launch(); CK(cudaDeviceSynchronize());
     long long h[148]; CK(cudaMemcpy(h,cyc,sizeof(h),cudaMemcpyDeviceToHost));
     double avg=0; for(int i=0;i<148;++i) avg+=h[i]; avg/=148;
-    printf("%s %s mask %-14s: %.3f clk/warp-instr/SM\n",w==0?"LDS.64 ":w==1?"LDS.32 ":"LDS.128",bc?"bcast ":"linear",mk.n,avg/(kIters*8.0*16));
+    printf("%s %s mask %-14s: %.3f clk/warp-instr/SM\n",w==0?"LDS.64 ":w==1?"LDS.32 ":"LDS.128",bc==0?"linear":bc==1?"bcast ":bc==2?"2 addr":"4 addr",mk.n,avg/(kIters*8.0*16));
   }
   return 0;
 }
