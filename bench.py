@@ -70,6 +70,22 @@ class ClockSampler(threading.Thread):
                 "samples": len(self.rows), "power_w_max": max(float(r[2]) for r in self.rows)}
 
 
+def reduce_times_max(times, device):
+    """Element-wise MAX of per-rank times over all ranks (the replicas run side by side: the job takes as long as its
+    slowest rank).  Identity when torch.distributed is not initialised or has one rank."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(times), dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t]
+
+
+def job_throughput(units_per_rank, world, ms):
+    """Whole-job units per second of `world` replicas that each processed `units_per_rank` in `ms` (weak scaling)."""
+    return world * units_per_rank / (ms * 1e-3)
+
+
 def nominal_cmacs(params, rec):
     """nominal complex MACs of one gridding pass = n_corr * n_pol * sum_k S_k^2 over kept visibilities."""
     keep = ~rec["drop"]
@@ -260,17 +276,14 @@ def run_ours(args):
     h2d = h_uvw.numel() * 4 + h_vis.numel() * 8 + h_wts.numel() * 4 + (h_a.numel() * 4 if h_a is not None else 0)
     d2h = h_out.numel() * 8 + h_grid.numel() * 8
 
-    times = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-    total_ms, e2e_ms = float(times[0]), float(times[1])
+    total_ms, e2e_ms = reduce_times_max([total_ms, e2e_ms], dev)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
     peaks, peaks_kind = load_peaks()
     ms_per_step = total_ms / args.steps
-    value = world * nvis / (ms_per_step * 1e-3)
+    value = job_throughput(nvis, world, ms_per_step)
     peak_tflops = N_SM * FP32_FMA_PER_CLK_SM * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 * 2 / 1e12
     achieved = 8.0 * cmacs / (kern["grid"] * 1e-3) / 1e12
     traffic = None                                  # DRAM bytes per launch of the gridding kernel, from the committed ncu capture
@@ -290,7 +303,7 @@ def run_ours(args):
                    "step": "imager_grid (index+sort+grid) + imager_degrid (index reused)",
                    "e2e_step": f"{nch} chunks: H2D uvw_k -> imager_index_k || H2D vis_k, weights_k -> imager_grid_k; D2H grid || imager_degrid_k -> D2H vis_k"},
         "clocks": sampler.summary(),
-        "e2e": {"value": world * nvis / (e2e_ms * 1e-3), "unit": "vis/s", "h2d_bytes_per_step": h2d,
+        "e2e": {"value": job_throughput(nvis, world, e2e_ms), "unit": "vis/s", "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms},
         "gpu_launches": launches,
         "roofline": {"bound": "alu", "kernel": "gridding (imager_grid, index reused)", "achieved": achieved,
