@@ -206,21 +206,58 @@ __device__ __forceinline__ uint32_t ctrl_variant(uint32_t ctrl) {
 
 // Hit counts per (gu, strip), visibility-centric: every kept visibility adds 1 to each strip its footprint meets
 // (about 4 atomics per visibility; sorted order makes neighbouring threads meet the same few counters in L2).
+#ifndef IMAGER_AGGREGATE
+#define IMAGER_AGGREGATE 1
+#endif
+// the strips a kept visibility meets: cell index of its t-th hit, t = 0 .. n - 1 (row-major over the strips)
+struct VisHits {
+    int64_t cell0;      // (gu, strip (sy0, sx0))
+    int nsx, n, x0, y0, sx0, sy0, S, subl, kset;
+};
+__device__ __forceinline__ VisHits vis_hits(const PlanArgs& a, const uint2 geo) {
+    VisHits v;
+    const int gx = (int)(geo.x & 0xffffu), gy = (int)(geo.x >> 16);
+    const int sub = (int)(geo.y & kSubMask);
+    v.kset = (int)(geo.y >> kSubBits);
+    const SetPlan sp = a.set_plan[v.kset];
+    v.S = a.set_support[v.kset];
+    const int h_lo = v.S / 2, group = sub / sp.group_slices;
+    v.subl = sub - group * sp.group_slices;
+    v.x0 = gx - h_lo;                                                  // footprint origin, inside the grid for kept ones
+    v.y0 = gy - h_lo;
+    v.sx0 = v.x0 / kStripW;
+    v.sy0 = v.y0 / kStripH;
+    v.nsx = (v.x0 + v.S - 1) / kStripW - v.sx0 + 1;
+    v.n = v.nsx * ((v.y0 + v.S - 1) / kStripH - v.sy0 + 1);
+    v.cell0 = (int64_t)(sp.gu_base + group) * a.g.n_strips + (int64_t)v.sy0 * a.g.strips_per_row + v.sx0;
+    return v;
+}
+
 __global__ void count_hits_kernel(const PlanArgs a, const int32_t* __restrict__ counters, int32_t* __restrict__ hits) {
     const Geometry& g = a.g;
     const int n_kept = counters[0];
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_kept; i += gridDim.x * blockDim.x) {
-        const uint2 geo = a.sgeo[i];
-        const int gx = (int)(geo.x & 0xffffu), gy = (int)(geo.x >> 16);
-        const int sub = (int)(geo.y & kSubMask), kset = (int)(geo.y >> kSubBits);
-        const SetPlan sp = a.set_plan[kset];
-        const int S = a.set_support[kset], h_lo = S / 2;
-        const int gu = sp.gu_base + sub / sp.group_slices;
-        const int x0 = gx - h_lo, y0 = gy - h_lo;                       // footprint origin, inside the grid for kept ones
-        const int sx0 = x0 / kStripW, sx1 = (x0 + S - 1) / kStripW, sy0 = y0 / kStripH, sy1 = (y0 + S - 1) / kStripH;
-        int32_t* base = hits + (int64_t)gu * g.n_strips;
-        for (int sy = sy0; sy <= sy1; ++sy)
-            for (int sx = sx0; sx <= sx1; ++sx) atomicAdd(base + sy * g.strips_per_row + sx, 1);
+    const int lane = threadIdx.x & 31;
+    // warp-uniform trip count: the lanes of a warp hold consecutive sorted visibilities, which mostly meet the same strips
+    for (int i0 = (blockIdx.x * blockDim.x + threadIdx.x) - lane; i0 < n_kept; i0 += gridDim.x * blockDim.x) {
+        const int i = i0 + lane;
+        VisHits v;
+        v.n = 0;
+        if (i < n_kept) v = vis_hits(a, a.sgeo[i]);
+#if IMAGER_AGGREGATE
+        const int n_max = __reduce_max_sync(0xffffffffu, v.n);
+        for (int t = 0; t < n_max; ++t) {
+            const bool on = t < v.n;
+            const int ty = on ? t / v.nsx : 0;
+            const long long cell = on ? v.cell0 + (int64_t)ty * g.strips_per_row + (t - ty * v.nsx) : -1ll - lane;
+            const unsigned peers = __match_any_sync(0xffffffffu, cell);         // lanes that meet the same (gu, strip)
+            if (on && lane == __ffs(peers) - 1) atomicAdd(hits + cell, __popc(peers));
+        }
+#else
+        for (int t = 0; t < v.n; ++t) {
+            const int ty = t / v.nsx;
+            atomicAdd(hits + v.cell0 + (int64_t)ty * g.strips_per_row + (t - ty * v.nsx), 1);
+        }
+#endif
     }
 }
 
@@ -236,26 +273,47 @@ __global__ void emit_hits_kernel(const PlanArgs a, const int32_t* __restrict__ c
                                  int32_t* __restrict__ cursor, uint2* __restrict__ hit_tmp) {
     const Geometry& g = a.g;
     const int n_kept = counters[0];
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_kept; i += gridDim.x * blockDim.x) {
-        const uint2 geo = a.sgeo[i];
-        const int gx = (int)(geo.x & 0xffffu), gy = (int)(geo.x >> 16);
-        const int sub = (int)(geo.y & kSubMask), kset = (int)(geo.y >> kSubBits);
-        const SetPlan sp = a.set_plan[kset];
-        const int S = a.set_support[kset], h_lo = S / 2;
-        const int group = sub / sp.group_slices, subl = sub - group * sp.group_slices;
-        const int gu = sp.gu_base + group;
-        const int x0 = gx - h_lo, y0 = gy - h_lo;
-        const int sx0 = x0 / kStripW, sx1 = (x0 + S - 1) / kStripW, sy0 = y0 / kStripH, sy1 = (y0 + S - 1) / kStripH;
-        const int slice_taps = sp.rows * sp.pitch;
-        for (int sy = sy0; sy <= sy1; ++sy)
-            for (int sx = sx0; sx <= sx1; ++sx) {
-                const int dx0 = sx * kStripW - x0, dy0 = sy * kStripH - y0;      // tap coordinates of the strip origin
-                const uint32_t ctrl = hit_ctrl(dx0, dy0, S, subl, sp.group_slices);
-                const int64_t cell = (int64_t)gu * g.n_strips + sy * g.strips_per_row + sx;
-                const int pos = atomicAdd(cursor + cell, 1);
-                const int tapoff = subl * slice_taps + (dy0 + kPadY) * sp.pitch + dx0 + kPadX;
+    const int lane = threadIdx.x & 31;
+    const unsigned lt_mask = (1u << lane) - 1u;
+    for (int i0 = (blockIdx.x * blockDim.x + threadIdx.x) - lane; i0 < n_kept; i0 += gridDim.x * blockDim.x) {
+        const int i = i0 + lane;
+        VisHits v;
+        v.n = 0;
+        int pitch = 0, slice_taps = 0, group_slices = 1;
+        if (i < n_kept) {
+            v = vis_hits(a, a.sgeo[i]);
+            const SetPlan sp = a.set_plan[v.kset];
+            pitch = sp.pitch;
+            slice_taps = sp.rows * sp.pitch;
+            group_slices = sp.group_slices;
+        }
+#if IMAGER_AGGREGATE
+        const int n_max = __reduce_max_sync(0xffffffffu, v.n);
+#else
+        const int n_max = v.n;
+#endif
+        for (int t = 0; t < n_max; ++t) {
+            const bool on = t < v.n;
+            const int ty = on ? t / v.nsx : 0, tx = t - ty * v.nsx;
+            const long long cell = on ? v.cell0 + (int64_t)ty * g.strips_per_row + tx : -1ll - lane;
+            int pos;
+#if IMAGER_AGGREGATE
+            const unsigned peers = __match_any_sync(0xffffffffu, cell);
+            const int leader = __ffs(peers) - 1;
+            int base = 0;
+            if (on && lane == leader) base = atomicAdd(cursor + cell, __popc(peers));
+            base = __shfl_sync(0xffffffffu, base, leader);
+            pos = base + __popc(peers & lt_mask);
+#else
+            pos = atomicAdd(cursor + cell, 1);
+#endif
+            if (on) {
+                const int dx0 = (v.sx0 + tx) * kStripW - v.x0, dy0 = (v.sy0 + ty) * kStripH - v.y0;   // taps of the strip origin
+                const uint32_t ctrl = hit_ctrl(dx0, dy0, v.S, v.subl, group_slices);
+                const int tapoff = v.subl * slice_taps + (dy0 + kPadY) * pitch + dx0 + kPadX;
                 hit_tmp[(int64_t)hit_start[cell] + pos] = make_uint2((uint32_t)i, (uint32_t)(tapoff + (int)kTapBias) | (ctrl << 24));
             }
+        }
     }
 }
 
