@@ -43,12 +43,33 @@ class ClockSampler(threading.Thread):
 
     def __init__(self, index=0):
         super().__init__(daemon=True)
-        self.rows, self.stop_flag, self.index = [], False, index
+        self.rows, self.stamps, self.stop_flag, self.index = [], [], False, index
+        self.t_begin, self.t_end = 0.0, float("inf")
         self.query = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
                       "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
                       "clocks_event_reasons.sw_power_cap")
 
+    def _nvml_loop(self):
+        """NVML directly (a query takes microseconds; nvidia-smi takes ~0.4 s per call on these boxes)."""
+        import pynvml
+        pynvml.nvmlInit()
+        h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+        get_reasons = getattr(pynvml, "nvmlDeviceGetCurrentClocksEventReasons", None) or pynvml.nvmlDeviceGetCurrentClocksThrottleReasons
+        bits = [0x8, 0x40, 0x20, 0x4]            # hw_slowdown, hw_thermal_slowdown, sw_thermal_slowdown, sw_power_cap
+        sm_max = pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM)
+        while not self.stop_flag:
+            r = int(get_reasons(h))
+            self.rows.append([str(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)), str(sm_max),
+                              str(pynvml.nvmlDeviceGetPowerUsage(h) / 1000.0)] + ["Active" if r & b else "Not Active" for b in bits])
+            self.stamps.append(time.perf_counter())
+            time.sleep(0.01)
+
     def run(self):
+        try:
+            self._nvml_loop()
+            return
+        except Exception:
+            pass                                  # no NVML binding: fall back to the nvidia-smi command line
         while not self.stop_flag:
             try:
                 out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.query}",
@@ -56,11 +77,14 @@ class ClockSampler(threading.Thread):
                 parts = [p.strip() for p in out.strip().split(",")]
                 if len(parts) >= 7:
                     self.rows.append(parts)
+                    self.stamps.append(time.perf_counter())
             except Exception:
                 pass
             time.sleep(0.05)
 
     def summary(self):
+        rows_in = [r for r, t in zip(self.rows, self.stamps) if self.t_begin <= t <= self.t_end]
+        self.rows = rows_in or self.rows            # samples taken while the timed loops ran (all of them if none fell inside)
         if not self.rows:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         sm = sorted(float(r[0]) for r in self.rows)
@@ -179,13 +203,17 @@ def run_ours(args):
             dist.barrier()
             torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
-        step()
-    barrier()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
+    for _ in range(max(args.warmup, 3)):
+        step()
+    t_wait = time.perf_counter()
+    while rank == 0 and not sampler.rows and time.perf_counter() - t_wait < 3.0:
+        step()                                  # untimed: keep the GPU under load until nvidia-smi has answered once
+    barrier()
     launches = 0
+    sampler.t_begin = time.perf_counter()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     barrier()
     for a, b in ev:
@@ -210,6 +238,7 @@ def run_ours(args):
         torch.cuda.synchronize()
         kern[name] = float(np.mean([a.elapsed_time(b) for a, b in es]))
     barrier()
+    sampler.t_end = time.perf_counter()
     sampler.stop_flag = True
 
     # end to end: pinned host buffers, H2D of the step's inputs and D2H of its results inside the timed region
