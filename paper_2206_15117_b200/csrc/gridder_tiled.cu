@@ -1,26 +1,30 @@
 // gridder_tiled.cu -- the output-stationary ("tiled") gridding and degridding kernels (hot-path steps A3 / A6) and
-// their work planner.
+// their work planner (part of A2).  DESIGN.md section 6.2.
 //
-// Why this shape: every complex MAC needs one 8-byte tap that no other MAC can share
-// (the tap index depends on visibility AND cell), and on sm_100a a warp-wide LDS.64 occupies the shared-memory
-// pipe for 2 clocks whatever its lane mask (measured), so the binding unit is LDS INSTRUCTIONS, not HBM and not
-// the FMA pipe (1 LDS.64 + 2 FFMA2 per 32 complex MACs = 49.6 % of the FP32 peak at best).  The kernels therefore
+// Why this shape: every complex MAC needs one 8-byte tap that no other MAC can share (the tap index depends on
+// visibility AND cell), and on sm_100a ANY shared-memory load of up to 8 bytes per lane occupies the LSU pipe for
+// 2.1 clocks per warp instruction whatever its lane mask or address pattern (profiles/r1_lds_mask_probe.md), so the
+// binding unit is shared-memory load INSTRUCTIONS, not HBM and not the FMA pipe (1 LDS.64 + 2 FFMA2 per 32 complex
+// MACs = 50 % of the FP32 peak at best).  The kernels therefore
 //   (1) keep grid cells in REGISTERS: a warp owns a 16 x 32 strip, its 8 x 4 lane block replicated 2 x 8 times
-//       ("slots": 16 cells per lane, packed FFMA2 accumulators);
+//       ("slots": 16 cells per lane), one packed accumulator per cell (complex MAC = two FFMA2 with operand modifiers);
 //   (2) keep one unit (kernel set x group of sub-cell slices x Mueller element) resident in SHARED memory, rows
 //       zero-padded by 3, columns by 7, pitched to 8 mod 16 taps: an 8 x 4 lane block reads conflict-free, and
 //       lanes beyond a footprint edge read zeros without any per-lane test;
 //   (3) replay precomputed HITS: a hit is one (visibility, strip) pair with the tap address of the strip origin
 //       and the range of slots its footprint meets.  The hit lists are built on the device when (uvw, a_index)
 //       are indexed and are cached while those do not change (IMAGER_REUSE_INDEX: every major cycle after the
-//       first).  A hit costs one broadcast LDS.128, one REDUX for its warp-uniform slot range, and a jump into
-//       straight-line code specialised for that range (1 LDS.64 + 2 FFMA2 per slot, nothing else);
+//       first).  Hits are replayed in runs of equal slot range: one REDUX + ballot per run, then per hit one broadcast
+//       LDS.128 (value and tap address, loaded a hit ahead) and straight-line code specialised for the range
+//       (1 LDS.64 + 2 FFMA2 per slot, nothing else);
 //   (4) gridding flushes a strip once per work item with red.global.add.v2.f32; degridding loads the strip once
-//       per item, reduces each hit's 32 partial sums in batches of 8 by a shuffle transpose and adds the result to
-//       the visibility with one red.global.add.v2.f32.
-// Work planning: item = up to kItemHits hits of one (geometry unit, strip); block = consecutive items of one
-// geometry unit with about kBlockHits hits, times one Mueller element (s, c); persistent CTAs pull blocks from a
-// global queue, their 16 warps pull items of the block from a shared counter.
+//       per item, writes each hit's 32 partial sums with one STS.64, sums 8 hits at a time by a transposed read and
+//       two shuffles, and adds the result to the visibility with one red.global.add.v2.f32.
+// Work planning (visibility-centric, warp-aggregated atomics): hits per (geometry unit, strip) are counted, scanned,
+// emitted and counting-sorted by slot-range variant; item = up to kItemHits hits of one (unit, strip); block =
+// consecutive items of one unit with about kBlockHits hits, times one Mueller element (s, c); persistent CTAs pull
+// blocks from a two-ended global queue (small blocks last), their warps pull items of the block from a shared counter.
+// IMAGER_PAIR = 1 builds the two-hits-per-warp experiment of gridder_pair.cuh instead of the kernels below.
 #include "common.cuh"
 
 namespace imager {
