@@ -89,14 +89,6 @@ struct Geometry {
     int N, O, nt, strips_per_row, n_strips, n_sets, n_gu, n_pol, n_corr;
 };
 
-__device__ __forceinline__ void ffma2(float2& d, const float2 a, const float2 b) {
-    unsigned long long dd = *reinterpret_cast<unsigned long long*>(&d);
-    asm("fma.rn.f32x2 %0, %1, %2, %0;"
-        : "+l"(dd)
-        : "l"(*reinterpret_cast<const unsigned long long*>(&a)), "l"(*reinterpret_cast<const unsigned long long*>(&b)));
-    d = *reinterpret_cast<float2*>(&dd);
-}
-
 __device__ __forceinline__ float2 lds64(uint32_t addr) {
     float2 v;
     asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
@@ -160,7 +152,6 @@ struct PlanArgs {
     const SetPlan* set_plan;
     const int32_t* gu_set;
     const int32_t* set_support;
-    const int32_t* bucket_offset;
     const uint2* sgeo;
 };
 
@@ -589,14 +580,6 @@ __device__ __forceinline__ uint32_t ctrl_slot_mask(uint32_t ctrl) {
     const uint32_t rows = (1u << jh) - (1u << jl);
     return ((ctrl & 0x40u) ? rows : 0u) | ((ctrl & 0x80u) ? rows << 8 : 0u);
 }
-
-// Shared by gridding and degridding: block / item queues and the staging of hit descriptors.
-// stage[lane] = {shared address of the strip-origin tap, value.x, value.y, sorted index}
-struct WarpCtx {
-    uint4* stage;
-    uint32_t tab_addr;
-    int lane, lx, ly;
-};
 
 template <int NC>
 __global__ void __launch_bounds__(kGridThreads, 1)
@@ -1034,7 +1017,6 @@ static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
     pa.set_plan = st->d_plan;
     pa.gu_set = st->d_gu_set;
     pa.set_support = pl->d_set_support;
-    pa.bucket_offset = pl->d_bucket_offset;
     pa.sgeo = st->d_sgeo;
     IMAGER_CUDA(cudaMemsetAsync(st->d_hits, 0, (n_cells + 1) * sizeof(int32_t), stream));
     count_hits_kernel<<<8 * kNumSMs, 256, 0, stream>>>(pa, pl->d_counters, st->d_hits);
