@@ -48,7 +48,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-PROBES = ["port_probe", "lds_mask_probe", "tmem_shape_probe"]
+PROBES = ["port_probe", "lds_mask_probe", "tmem_shape_probe", "lsu_mix_probe"]
 
 
 def build_probe() -> list:
