@@ -108,6 +108,84 @@ __global__ void sorted_geo_kernel(const int32_t* __restrict__ counters, const in
     }
 }
 
+// ---- exact pre-summation of duplicates (S16 / R16: "pre-summing duplicate (cell, sub-cell, plane, A-plane)
+// visibilities is exact algebra") -----------------------------------------------------------------------------
+// Visibilities with the same (kernel set, cell, sub-cell) use the same taps on the same cells: gridding grids the SUM of
+// their weighted values once, degridding predicts one value and copies it.  rep[i] = the smallest sorted index with
+// i's geometry among the kDedupeChunk consecutive sorted visibilities of i's chunk (equal geometries are neighbours in
+// the sorted order up to the tile's other visibilities; a duplicate in another chunk is simply not merged).
+#ifndef IMAGER_DEDUPE
+#define IMAGER_DEDUPE 1
+#endif
+constexpr int kDedupeChunk = 4096, kDedupeSlots = 8192;          // shared hash table: load factor <= 0.5
+constexpr int kDedupeSmem = kDedupeSlots * 12;
+constexpr uint32_t kMergedFlag = 0x8000u;                       // bit 15 of sgeo.x (gx < 2^15): merged into another one
+constexpr int kDedupeThreads = 256, kDedupePer = kDedupeChunk / kDedupeThreads;
+// Fused with the sorted-geometry pass: one CTA builds sgeo for kDedupeChunk consecutive sorted visibilities, finds their
+// representatives through a shared hash table (min sorted index per geometry) and flags the merged ones.
+__global__ void __launch_bounds__(kDedupeThreads) sorted_geo_dedupe_kernel(const int32_t* __restrict__ counters,
+                                                                           const int32_t* __restrict__ perm,
+                                                                           const imager_record* __restrict__ rec, int O,
+                                                                           uint2* __restrict__ sgeo, int32_t* __restrict__ rep) {
+    extern __shared__ __align__(16) unsigned char dedupe_smem[];
+    unsigned long long* s_key = reinterpret_cast<unsigned long long*>(dedupe_smem);
+    int32_t* s_idx = reinterpret_cast<int32_t*>(dedupe_smem + kDedupeSlots * sizeof(unsigned long long));
+    const int n_kept = counters[0];
+    const int c0 = blockIdx.x * kDedupeChunk;
+    if (c0 >= n_kept) return;
+    const int c1 = min(n_kept, c0 + kDedupeChunk);
+    uint2 geo[kDedupePer];
+#pragma unroll
+    for (int j = 0; j < kDedupePer; ++j) {
+        const int i = c0 + j * kDedupeThreads + threadIdx.x;
+        if (i < c1) {
+            const imager_record r = rec[perm[i]];
+            geo[j] = make_uint2((uint32_t)r.gx | ((uint32_t)r.gy << 16),
+                                (((r.sub >> 8) & 255u) * O + (r.sub & 255u)) | ((uint32_t)r.kset << kSubBits));
+        }
+    }
+    for (int q = threadIdx.x; q < kDedupeSlots; q += blockDim.x) {
+        s_key[q] = ~0ull;                                               // no geometry has all bits set (kset < 2^18)
+        s_idx[q] = 0x7fffffff;
+    }
+    __syncthreads();
+    for (int pass = 0; pass < 2; ++pass) {                              // 0: insert (min index per geometry), 1: look up
+#pragma unroll
+        for (int j = 0; j < kDedupePer; ++j) {
+            const int i = c0 + j * kDedupeThreads + threadIdx.x;
+            if (i >= c1) continue;
+            const unsigned long long key = ((unsigned long long)geo[j].y << 32) | geo[j].x;
+            uint32_t h = (uint32_t)((key * 0x9E3779B97F4A7C15ull) >> 51) & (kDedupeSlots - 1);
+            for (;;) {
+                const unsigned long long old = pass == 0 ? atomicCAS(&s_key[h], ~0ull, key) : s_key[h];
+                if (old == key || (pass == 0 && old == ~0ull)) break;
+                h = (h + 1) & (kDedupeSlots - 1);
+            }
+            if (pass == 0) {
+                atomicMin(&s_idx[h], i);
+            } else {
+                const int r = s_idx[h];
+                rep[i] = r;
+                sgeo[i] = make_uint2(geo[j].x | (r != i ? kMergedFlag : 0u), geo[j].y);
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// sval[rep] += sval[i] for every merged visibility i (after gather_values_kernel)
+template <int NC>
+__global__ void accumulate_duplicates_kernel(const int32_t* __restrict__ counters, const int32_t* __restrict__ rep,
+                                             float2* __restrict__ sval) {
+    const int n_kept = counters[0];
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_kept; i += gridDim.x * blockDim.x) {
+        const int r = rep[i];
+        if (r == i) continue;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) atomicAdd(&sval[(int64_t)r * NC + c], sval[(int64_t)i * NC + c]);
+    }
+}
+
 // sorted-order weighted visibilities  w_kc * V_kc
 template <int NC>
 __global__ void gather_values_kernel(const int32_t* __restrict__ counters, const int32_t* __restrict__ perm,
@@ -129,13 +207,15 @@ __global__ void gather_values_kernel(const int32_t* __restrict__ counters, const
 // the prediction is subtracted from what vis_out holds (V - V_model, the major-cycle update)
 template <int NC>
 __global__ void scatter_values_kernel(int64_t nvis, const int32_t* __restrict__ counters, const int32_t* __restrict__ perm,
-                                      const float2* __restrict__ sval, int residual, float2* __restrict__ vis_out) {
+                                      const int32_t* __restrict__ rep, const float2* __restrict__ sval, int residual,
+                                      float2* __restrict__ vis_out) {
     const int n_kept = counters[0];
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvis; i += (int64_t)gridDim.x * blockDim.x) {
         const int64_t k = perm[i];
+        const int64_t src = (rep && i < n_kept) ? rep[i] : i;              // merged duplicates share one prediction
 #pragma unroll
         for (int c = 0; c < NC; ++c) {
-            const float2 m = i < n_kept ? sval[i * NC + c] : make_float2(0.f, 0.f);
+            const float2 m = i < n_kept ? sval[src * NC + c] : make_float2(0.f, 0.f);
             float2* o = vis_out + k * NC + c;
             *o = residual ? make_float2(o->x - m.x, o->y - m.y) : m;
         }
@@ -211,7 +291,7 @@ struct VisHits {
 };
 __device__ __forceinline__ VisHits vis_hits(const PlanArgs& a, const uint2 geo) {
     VisHits v;
-    const int gx = (int)(geo.x & 0xffffu), gy = (int)(geo.x >> 16);
+    const int gx = (int)(geo.x & 0x7fffu), gy = (int)(geo.x >> 16);           // bit 15: merged flag
     const int sub = (int)(geo.y & kSubMask);
     v.kset = (int)(geo.y >> kSubBits);
     const SetPlan sp = a.set_plan[v.kset];
@@ -237,7 +317,10 @@ __global__ void count_hits_kernel(const PlanArgs a, const int32_t* __restrict__ 
         const int i = i0 + lane;
         VisHits v;
         v.n = 0;
-        if (i < n_kept) v = vis_hits(a, a.sgeo[i]);
+        if (i < n_kept) {
+            const uint2 geo = a.sgeo[i];
+            if (!(geo.x & 0x8000u)) v = vis_hits(a, geo);                      // merged duplicates have no hits of their own
+        }
 #if IMAGER_AGGREGATE
         const int n_max = __reduce_max_sync(0xffffffffu, v.n);
         for (int t = 0; t < n_max; ++t) {
@@ -275,8 +358,10 @@ __global__ void emit_hits_kernel(const PlanArgs a, const int32_t* __restrict__ c
         VisHits v;
         v.n = 0;
         int pitch = 0, slice_taps = 0, group_slices = 1;
-        if (i < n_kept) {
-            v = vis_hits(a, a.sgeo[i]);
+        uint2 geo = make_uint2(0x8000u, 0u);
+        if (i < n_kept) geo = a.sgeo[i];
+        if (!(geo.x & 0x8000u)) {
+            v = vis_hits(a, geo);
             const SetPlan sp = a.set_plan[v.kset];
             pitch = sp.pitch;
             slice_taps = sp.rows * sp.pitch;
@@ -878,6 +963,7 @@ struct TiledState {
     int64_t cap_hits = 0, cap_items = 0, cap_blocks = 0, cap_tmp = 0;
     int32_t* h_totals = nullptr;          // pinned [2]
     uint2* d_sgeo = nullptr;
+    int32_t* d_rep = nullptr;             // [max_nvis] representative of every sorted visibility (IMAGER_DEDUPE)
     float2* d_sval = nullptr;
     int64_t plan_epoch = -1;
     int32_t blocks_cap = 0;               // the two-ended block queue lives in d_blocks[0 .. blocks_cap)
@@ -965,6 +1051,7 @@ void tiled_release(imager_plan* pl) {
     cudaFree(st->d_item_rec);
     cudaFree(st->d_blocks);
     cudaFree(st->d_sgeo);
+    cudaFree(st->d_rep);
     cudaFree(st->d_sval);
     if (st->h_totals) cudaFreeHost(st->h_totals);
     delete st;
@@ -1002,6 +1089,10 @@ static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
         IMAGER_CUDA(cudaMalloc(&st->d_cursor, (n_cells + 1) * sizeof(int32_t)));
         IMAGER_CUDA(cudaMalloc(&st->d_scan_tmp, tmp_len * sizeof(int32_t)));
         IMAGER_CUDA(cudaMalloc(&st->d_sgeo, mv * sizeof(uint2)));
+#if IMAGER_DEDUPE
+        IMAGER_CUDA(cudaMalloc(&st->d_rep, mv * sizeof(int32_t)));
+        IMAGER_CUDA(cudaFuncSetAttribute(sorted_geo_dedupe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kDedupeSmem));
+#endif
         IMAGER_CUDA(cudaMalloc(&st->d_sval, mv * pl->p.n_corr * sizeof(float2)));
         IMAGER_CUDA(cudaMallocHost(&st->h_totals, 2 * sizeof(int32_t)));
         IMAGER_CUDA(cudaFuncSetAttribute(IMAGER_GRID_KERNEL<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
@@ -1010,8 +1101,13 @@ static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
         IMAGER_CUDA(cudaFuncSetAttribute(IMAGER_DEGRID_KERNEL<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
     }
     if (st->plan_epoch == pl->index_epoch) return 0;
+#if IMAGER_DEDUPE
+    sorted_geo_dedupe_kernel<<<(unsigned)((pl->indexed_nvis + kDedupeChunk - 1) / kDedupeChunk), kDedupeThreads, kDedupeSmem, stream>>>(
+        pl->d_counters, pl->d_perm[pl->sorted_buf], pl->d_rec, pl->p.oversample, st->d_sgeo, st->d_rep);
+#else
     sorted_geo_kernel<<<4 * kNumSMs, 256, 0, stream>>>(pl->d_counters, pl->d_perm[pl->sorted_buf], pl->d_rec,
                                                        pl->p.oversample, st->d_sgeo);
+#endif
     PlanArgs pa;
     pa.g = g;
     pa.set_plan = st->d_plan;
@@ -1099,6 +1195,11 @@ int launch_grid_tiled(imager_plan* pl, int64_t nvis, const float2* vis, const fl
         gather_values_kernel<1><<<gb, 256, 0, stream>>>(pl->d_counters, pl->d_perm[pl->sorted_buf], vis, weights, st->d_sval);
     else
         gather_values_kernel<4><<<gb, 256, 0, stream>>>(pl->d_counters, pl->d_perm[pl->sorted_buf], vis, weights, st->d_sval);
+    if (st->d_rep) {
+        if (pl->p.n_corr == 1) accumulate_duplicates_kernel<1><<<gb, 256, 0, stream>>>(pl->d_counters, st->d_rep, st->d_sval);
+        else accumulate_duplicates_kernel<4><<<gb, 256, 0, stream>>>(pl->d_counters, st->d_rep, st->d_sval);
+        pl->last_launches += 1;
+    }
     IMAGER_CUDA(cudaMemsetAsync(pl->d_counters + 8, 0, sizeof(int32_t), stream));
     TiledArgs a;
     fill_args(pl, st, a, pl->d_tab_grid);
@@ -1125,10 +1226,10 @@ int launch_degrid_tiled(imager_plan* pl, int64_t nvis, const float2* grid, float
     const unsigned gb = 4 * kNumSMs;
     if (nc == 1) {
         IMAGER_DEGRID_KERNEL<1><<<kNumSMs, kTiledThreads, smem, stream>>>(a, grid, st->d_sval);
-        scatter_values_kernel<1><<<gb, 256, 0, stream>>>(nvis, pl->d_counters, pl->d_perm[pl->sorted_buf], st->d_sval, residual, vis_out);
+        scatter_values_kernel<1><<<gb, 256, 0, stream>>>(nvis, pl->d_counters, pl->d_perm[pl->sorted_buf], st->d_rep, st->d_sval, residual, vis_out);
     } else {
         IMAGER_DEGRID_KERNEL<4><<<kNumSMs, kTiledThreads, smem, stream>>>(a, grid, st->d_sval);
-        scatter_values_kernel<4><<<gb, 256, 0, stream>>>(nvis, pl->d_counters, pl->d_perm[pl->sorted_buf], st->d_sval, residual, vis_out);
+        scatter_values_kernel<4><<<gb, 256, 0, stream>>>(nvis, pl->d_counters, pl->d_perm[pl->sorted_buf], st->d_rep, st->d_sval, residual, vis_out);
     }
     pl->last_launches += 2;
     IMAGER_CUDA(cudaGetLastError());
