@@ -246,3 +246,48 @@ def test_degrid_residual_flag(torch_cuda, oracle_lib, flags):
     assert np.array_equal(got[rec["drop"]], vis[rec["drop"]])             # dropped: predicted 0, left as they are
     ok = refd["norm"] > 0
     assert float(np.max(np.abs(got[ok] - want[ok]) / (refd["norm"][ok] + np.abs(vis[ok])))) <= TOL
+
+
+@pytest.mark.parametrize("case", ["wproj", "awproj"])
+def test_duplicate_visibilities_are_presummed_exactly(torch_cuda, oracle_lib, case):
+    """Visibilities with the same (kernel set, cell, sub-cell) are merged by the library (their weighted values summed
+    before gridding, one prediction copied to all of them in degridding): results must stay those of the oracle, which
+    treats every visibility on its own.  Half of the inputs here are exact duplicates in uvw with their own values,
+    weights (some zero) and, for the residual, observed visibilities."""
+    torch = torch_cuda
+    from paper_2206_15117_b200 import Plan, DEGRID_RESIDUAL
+    params = CASES[case]()
+    n0 = 3000
+    uvw, vis, wts, a = random_vis(params, n0, seed=77, frac=0.45, a_planes=params["n_aplanes"] > 1)
+    rng = np.random.default_rng(78)
+    pick = rng.integers(0, n0, 3000)
+    uvw = np.concatenate([uvw, uvw[pick]])
+    a = None if a is None else np.concatenate([a, a[pick]])
+    extra = (rng.standard_normal((3000,) + vis.shape[1:]) + 1j * rng.standard_normal((3000,) + vis.shape[1:])).astype(np.complex64)
+    vis = np.concatenate([vis, extra])
+    wts = np.concatenate([wts, rng.random((3000,) + wts.shape[1:]).astype(np.float32)])
+    wts[::13] = 0.0
+    nvis = uvw.shape[0]
+    _, _, flat, offs = oracle_tables(params)
+    rec = oidx.index_visibilities(uvw, a, params)
+    ref = og.grid(rec, vis, wts, flat, offs, params)
+    n, npol, nc = params["grid_size"], params["n_pol"], params["n_corr"]
+    with Plan(params, nvis, user_tables=flat) as plan:
+        d_uvw, d_vis, d_wts, d_a = _to_dev(torch, uvw, vis, wts, a)
+        grid = torch.zeros((npol, n, n), dtype=torch.complex64, device="cuda")
+        plan.grid(d_uvw, d_vis, d_wts, grid, d_a)
+        out = torch.empty((nvis, nc), dtype=torch.complex64, device="cuda")
+        plan.degrid(d_uvw, grid, out, d_a, flags=1)
+        res = d_vis.clone()
+        plan.degrid(d_uvw, grid, res, d_a, flags=1 | DEGRID_RESIDUAL)
+        torch.cuda.synchronize()
+        g = grid.cpu().numpy()
+        assert grid_error(g, ref) <= TOL
+        refd = og.degrid(rec, g, flat, offs, params)
+        v = out.cpu().numpy()
+        assert vis_error(v, refd, rec["drop"]) <= TOL
+        ok = refd["norm"] > 0
+        same = ok[n0:] & ok[pick]                  # a duplicate gets its original's prediction (bit-equal when merged)
+        assert float(np.max(np.abs(v[n0:][same] - v[pick][same]) / refd["norm"][n0:][same])) <= TOL
+        want = vis.astype(np.complex128) - refd["vis"]
+        assert float(np.max(np.abs(res.cpu().numpy()[ok] - want[ok]) / (refd["norm"][ok] + np.abs(vis[ok])))) <= TOL
