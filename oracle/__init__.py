@@ -19,6 +19,6 @@ Modules
   gridder.py  ctypes wrapper of gridder.c
   imaging.py  O0/O7 grid<->image DFT with taper correction, direct DFT, Eq. 1 mosaic weighting
 
-Pins (tests/test_oracle_*.py, `-m "not gpu"`): P1-P12 of DESIGN.md.  Parity unpinned: see DESIGN.md
+Pins (tests/test_oracle_*.py, `-m "not gpu"`): P1-P14 of DESIGN.md.  Parity unpinned: see DESIGN.md
 "Parity unpinned" (config-level choices only: support schedule, PA binning, channel width, latitude).
 """

@@ -4,7 +4,7 @@ The product is `libimager.so` (CUDA, sm_100a; C-ABI in include/imager.h).  This 
 binding: the four hot-path calls keep their C names.  Nothing here computes anything on the CPU.
 """
 from .binding import (ImagerError, Plan, load_library, MODE_DELTA, MODE_PSWF, MODE_WPROJ, MODE_AWPROJ_ADJOINT,
-                      MODE_AWPROJ_PAPER, MODE_MOSAIC_PB, MODE_USER, REUSE_INDEX, PATH_REFERENCE, PATH_SMEM, PATH_TMEM, DEGRID_RESIDUAL, EXPORTS)
+                      MODE_AWPROJ_PAPER, MODE_MOSAIC_PB, MODE_USER, REUSE_INDEX, PATH_REFERENCE, DEGRID_RESIDUAL, EXPORTS)
 
 
 def imager_plan_create(params: dict, max_nvis: int, user_tables=None, user_tables_degrid=None, stream=None) -> Plan:

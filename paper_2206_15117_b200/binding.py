@@ -18,8 +18,6 @@ LIB_PATH = os.path.join(_HERE, "libimager.so")
 MODE_DELTA, MODE_PSWF, MODE_WPROJ, MODE_AWPROJ_ADJOINT, MODE_AWPROJ_PAPER, MODE_MOSAIC_PB, MODE_USER = range(7)
 REUSE_INDEX = 1
 PATH_REFERENCE = 2
-PATH_SMEM = 4
-PATH_TMEM = 8
 DEGRID_RESIDUAL = 16
 
 EXPORTS = ("imager_plan_create", "imager_index", "imager_grid", "imager_degrid", "imager_plan_destroy",

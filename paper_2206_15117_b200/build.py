@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libimager.so")
-SOURCES = ["api.cu", "index_sort.cu", "gridder_ref.cu", "gridder_tiled.cu", "gridder_tmem.cu", "tables.cu", "transform.cu"]
+SOURCES = ["api.cu", "index_sort.cu", "gridder_ref.cu", "gridder_tiled.cu", "tables.cu", "transform.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC",
               "-Xptxas", "-v"]
 
@@ -48,23 +48,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
-PROBES = ["port_probe", "lds_mask_probe", "tmem_shape_probe", "lsu_mix_probe"]
-
-
-def build_probe() -> list:
-    """The micro-benchmarks quoted in DESIGN.md / profiles/r1_*_probe.md (standalone executables next to the library)."""
-    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    out = []
-    for name in PROBES:
-        exe = os.path.join(HERE, name)
-        subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
-                               os.path.join(CSRC, name + ".cu"), "-o", exe])
-        out.append(exe)
-    return out
-
-
 if __name__ == "__main__":
-    if "--probe" in sys.argv:
-        print(build_probe())
-    else:
-        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

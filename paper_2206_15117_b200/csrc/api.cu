@@ -71,7 +71,6 @@ static void free_plan(imager_plan* pl) {
     cudaFree(pl->d_items);
     destroy_transform(pl);
     tiled_release(pl);
-    tmem_release(pl);
     delete pl;
 }
 
@@ -197,8 +196,6 @@ extern "C" int imager_grid(imager_plan* plan, int64_t nvis, const float* uvw, co
     if (rc) return rc;
     rc = launch_sum_weights(plan, nvis, weights, sum_weights, st);
     if (rc) return rc;
-    if ((flags & IMAGER_PATH_TMEM) && !(flags & IMAGER_PATH_REFERENCE) && tmem_supported(plan))
-        return launch_grid_tmem(plan, nvis, (const float2*)vis, weights, (float2*)grid, st);
     if (!(flags & IMAGER_PATH_REFERENCE) && tiled_supported(plan))
         return launch_grid_tiled(plan, nvis, (const float2*)vis, weights, (float2*)grid, st);
     return launch_grid_reference(plan, nvis, (const float2*)vis, weights, (float2*)grid, nullptr, st);

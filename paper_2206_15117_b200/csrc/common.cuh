@@ -53,7 +53,6 @@ struct imager_plan {
     bool index_valid = false;
     int64_t index_epoch = 0;             // bumped by every re-indexing
     void* tiled = nullptr;               // gridder_tiled.cu state (TiledState*)
-    void* tmem = nullptr;                // gridder_tmem.cu state (tm::TmState*)
 
     // tiled path work list
     int32_t* d_items = nullptr;          // [max_items][4]
@@ -90,12 +89,6 @@ int launch_grid_tiled(imager_plan* pl, int64_t nvis, const float2* vis, const fl
 int launch_degrid_tiled(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, int residual, cudaStream_t st);
 void tiled_release(imager_plan* pl);
 int tiled_prepare(imager_plan* pl, int64_t nvis, cudaStream_t st);
-
-// gridder_tmem.cu
-bool tmem_supported(const imager_plan* pl);
-int launch_grid_tmem(imager_plan* pl, int64_t nvis, const float2* vis, const float* weights, float2* grid, cudaStream_t st);
-int launch_degrid_tmem(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, cudaStream_t st);
-void tmem_release(imager_plan* pl);
 
 // tables.cu
 int build_tables(imager_plan* pl, const imager_params* user, cudaStream_t st);

@@ -24,23 +24,12 @@
 // emitted and counting-sorted by slot-range variant; item = up to kItemHits hits of one (unit, strip); block =
 // consecutive items of one unit with about kBlockHits hits, times one Mueller element (s, c); persistent CTAs pull
 // blocks from a two-ended global queue (small blocks last), their warps pull items of the block from a shared counter.
-// IMAGER_PAIR = 1 builds the two-hits-per-warp experiment of gridder_pair.cuh instead of the kernels below.
 #include "common.cuh"
 
 namespace imager {
 
-// IMAGER_PAIR = 1: TWO hits per warp instruction: each half-warp is a 4 x 4 lane block working on its own hit of a
-// 16 x 16 strip (4 x 4 slots); see gridder_pair.cuh.  IMAGER_PAIR = 0: one hit per warp, 8 x 4 lane block, 16 x 32 strips.
-#ifndef IMAGER_PAIR
-#define IMAGER_PAIR 0
-#endif
-#if IMAGER_PAIR
-constexpr int kLaneW = 4, kLaneH = 4;                 // lane block of a half-warp
-constexpr int kNX = 4, kNY = 4;                       // replications: strip = 16 x 16 cells
-#else
 constexpr int kLaneW = 8, kLaneH = 4;                 // lane block
 constexpr int kNX = 2, kNY = 8;                       // replications: strip = 16 x 32 cells
-#endif
 constexpr int kStripW = kLaneW * kNX, kStripH = kLaneH * kNY;
 constexpr int kPadY = kLaneH - 1, kPadX = kLaneW - 1;
 #ifndef IMAGER_DEGRID_THREADS
@@ -235,27 +224,6 @@ struct PlanArgs {
     const uint2* sgeo;
 };
 
-#if IMAGER_PAIR
-// ctrl byte of a hit: x-slots il .. ih-1 and y-slots jl .. jh-1 of the strip meet the footprint:
-// il | (ih - 1) << 2 | jl << 4 | (jh - 1) << 6   (dx0, dy0: tap coordinates of the strip origin)
-__device__ __forceinline__ uint32_t hit_ctrl(int dx0, int dy0, int S, int sub, int group_slices) {
-    const int il = (dx0 + kPadX < 0) ? (-dx0) / kLaneW : 0;
-    const int ih = min(kNX, (S - 1 - dx0) / kLaneW + 1);
-    const int jl = (dy0 + kPadY < 0) ? (-dy0) / kLaneH : 0;
-    const int jh = min(kNY, (S - 1 - dy0) / kLaneH + 1);
-    return (uint32_t)il | ((uint32_t)(ih - 1) << 2) | ((uint32_t)jl << 4) | ((uint32_t)(jh - 1) << 6);
-}
-
-// dense variant number of a ctrl byte: 10 x-ranges x 10 y-ranges
-#define IMAGER_R4(L, H1) ((L) * 4 - ((L) * ((L) - 1)) / 2 + (H1) - (L))
-#define IMAGER_VARIANT(IL, IH1, JL, JH1) (IMAGER_R4(IL, IH1) * 10 + IMAGER_R4(JL, JH1))
-constexpr int kVariants = 100;
-
-__device__ __forceinline__ uint32_t ctrl_variant(uint32_t ctrl) {
-    const int il = (int)(ctrl & 3u), ih1 = (int)((ctrl >> 2) & 3u), jl = (int)((ctrl >> 4) & 3u), jh1 = (int)(ctrl >> 6);
-    return (uint32_t)IMAGER_VARIANT(il, ih1, jl, jh1);
-}
-#else
 // ctrl byte of a candidate against a strip, or 0 if it is no hit (a hit always has bit 6 or 7 set)
 __device__ __forceinline__ uint32_t hit_ctrl(int dx0, int dy0, int S, int sub, int group_slices) {
     const bool hit = (dx0 + kStripW > 0) && (dx0 < S) && (dy0 + kStripH > 0) && (dy0 < S) &&
@@ -277,7 +245,6 @@ __device__ __forceinline__ uint32_t ctrl_variant(uint32_t ctrl) {
     return (uint32_t)IMAGER_VARIANT(h, jl, jh1);
 }
 
-#endif
 
 // Hit counts per (gu, strip), visibility-centric: every kept visibility adds 1 to each strip its footprint meets
 // (about 4 atomics per visibility; sorted order makes neighbouring threads meet the same few counters in L2).
@@ -600,7 +567,6 @@ __device__ __forceinline__ void ffma2p(u64& d, u64 a, u64 b) { asm("fma.rn.f32x2
 __device__ __forceinline__ void cmac_re(u64& acc, float2 t, float vr) { ffma2p(acc, pack2(t.x, t.y), pack2(vr, vr)); }
 __device__ __forceinline__ void cmac_im(u64& acc, float2 t, float vi) { ffma2p(acc, pack2(t.y, t.x), pack2(-vi, vi)); }
 
-#if !IMAGER_PAIR
 // A run: `cnt` consecutive staged hits with the same slot range.  A hit's descriptor {value.x, value.y, tap address, -}
 // is ONE broadcast LDS.128 (one wavefront), loaded a hit ahead; `d` carries the prefetched descriptor across runs.
 template <int H, int JL, int JH>
@@ -764,7 +730,6 @@ grid_tiled_kernel(const TiledArgs a, const float2* __restrict__ sval, float2* __
     }
 }
 
-#endif  // !IMAGER_PAIR
 
 // ---- degridding ------------------------------------------------------------------------------------------
 // Same hits, same ownership: the warp holds its strip of the grid in registers; a hit's lanes accumulate
@@ -786,7 +751,6 @@ __device__ __forceinline__ u64 add2p(u64 a, u64 b) {
     return r;
 }
 
-#if !IMAGER_PAIR
 template <int H, int JL, int JH>
 __device__ __forceinline__ void degrid_run(const float2 (&G0)[kNY], const float2 (&G1)[kNY], uint32_t desc_addr, int cnt,
                                            uint32_t red_addr, const uint32_t lane_off, const uint32_t (&step)[kNY]) {
@@ -934,16 +898,7 @@ degrid_tiled_kernel(const TiledArgs a, const float2* __restrict__ grid, float2* 
     }
 }
 
-#endif  // !IMAGER_PAIR
 
-#if IMAGER_PAIR
-#include "gridder_pair.cuh"
-#define IMAGER_GRID_KERNEL grid_pair_kernel
-#define IMAGER_DEGRID_KERNEL degrid_pair_kernel
-#else
-#define IMAGER_GRID_KERNEL grid_tiled_kernel
-#define IMAGER_DEGRID_KERNEL degrid_tiled_kernel
-#endif
 
 // ---- host side -------------------------------------------------------------------------------------------
 
@@ -972,13 +927,9 @@ struct TiledState {
 };
 
 // taps per padded table row: >= S + 2 kPadX and such that the lane block of a half-warp wavefront reads conflict-free
-// (8 x 2 lanes: 8 mod 16; 4 x 4 lanes: 4 mod 8)
+// (8 x 2 lanes: 8 mod 16)
 static int table_pitch(int S) {
-#if IMAGER_PAIR
-    return ((S + 2 * kPadX + 3) / 8) * 8 + 4;
-#else
     return ((S + 2 * kPadX + 7) / 16) * 16 + 8;
-#endif
 }
 
 bool tiled_supported(const imager_plan* pl) {
@@ -1095,10 +1046,10 @@ static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
 #endif
         IMAGER_CUDA(cudaMalloc(&st->d_sval, mv * pl->p.n_corr * sizeof(float2)));
         IMAGER_CUDA(cudaMallocHost(&st->h_totals, 2 * sizeof(int32_t)));
-        IMAGER_CUDA(cudaFuncSetAttribute(IMAGER_GRID_KERNEL<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
-        IMAGER_CUDA(cudaFuncSetAttribute(IMAGER_GRID_KERNEL<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
-        IMAGER_CUDA(cudaFuncSetAttribute(IMAGER_DEGRID_KERNEL<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
-        IMAGER_CUDA(cudaFuncSetAttribute(IMAGER_DEGRID_KERNEL<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
+        IMAGER_CUDA(cudaFuncSetAttribute(grid_tiled_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
+        IMAGER_CUDA(cudaFuncSetAttribute(grid_tiled_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
+        IMAGER_CUDA(cudaFuncSetAttribute(degrid_tiled_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
+        IMAGER_CUDA(cudaFuncSetAttribute(degrid_tiled_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
     }
     if (st->plan_epoch == pl->index_epoch) return 0;
 #if IMAGER_DEDUPE
@@ -1204,9 +1155,9 @@ int launch_grid_tiled(imager_plan* pl, int64_t nvis, const float2* vis, const fl
     TiledArgs a;
     fill_args(pl, st, a, pl->d_tab_grid);
     if (pl->p.n_corr == 1)
-        IMAGER_GRID_KERNEL<1><<<kNumSMs, kGridThreads, st->smem_bytes - kStageBytes + kGridStageBytes, stream>>>(a, st->d_sval, grid);
+        grid_tiled_kernel<1><<<kNumSMs, kGridThreads, st->smem_bytes - kStageBytes + kGridStageBytes, stream>>>(a, st->d_sval, grid);
     else
-        IMAGER_GRID_KERNEL<4><<<kNumSMs, kGridThreads, st->smem_bytes - kStageBytes + kGridStageBytes, stream>>>(a, st->d_sval, grid);
+        grid_tiled_kernel<4><<<kNumSMs, kGridThreads, st->smem_bytes - kStageBytes + kGridStageBytes, stream>>>(a, st->d_sval, grid);
     pl->last_launches += 2;
     IMAGER_CUDA(cudaGetLastError());
     return 0;
@@ -1225,10 +1176,10 @@ int launch_degrid_tiled(imager_plan* pl, int64_t nvis, const float2* grid, float
     const int smem = st->smem_bytes + kRedBytes;
     const unsigned gb = 4 * kNumSMs;
     if (nc == 1) {
-        IMAGER_DEGRID_KERNEL<1><<<kNumSMs, kTiledThreads, smem, stream>>>(a, grid, st->d_sval);
+        degrid_tiled_kernel<1><<<kNumSMs, kTiledThreads, smem, stream>>>(a, grid, st->d_sval);
         scatter_values_kernel<1><<<gb, 256, 0, stream>>>(nvis, pl->d_counters, pl->d_perm[pl->sorted_buf], st->d_rep, st->d_sval, residual, vis_out);
     } else {
-        IMAGER_DEGRID_KERNEL<4><<<kNumSMs, kTiledThreads, smem, stream>>>(a, grid, st->d_sval);
+        degrid_tiled_kernel<4><<<kNumSMs, kTiledThreads, smem, stream>>>(a, grid, st->d_sval);
         scatter_values_kernel<4><<<gb, 256, 0, stream>>>(nvis, pl->d_counters, pl->d_perm[pl->sorted_buf], st->d_rep, st->d_sval, residual, vis_out);
     }
     pl->last_launches += 2;

@@ -1,4 +1,4 @@
-"""Pins for oracle steps O4/O5/O7 (gridding, degridding, imaging): P1, P2, P3, P4, P6, P9, P11."""
+"""Pins for oracle steps O4/O5/O7 (gridding, degridding, imaging): P1, P2, P3, P4, P6, P9, P11, P13."""
 import numpy as np
 
 from oracle import index as oidx, kernels as ok, gridder as og, imaging as oi
@@ -181,3 +181,66 @@ def test_P11_identity_mueller_is_four_single_pol_runs(oracle_lib):
     scale = mix[0, 0]                                              # global normalisation makes element (0,0) unity
     expect = np.einsum("sc,cyx->syx", mix / scale, singles)
     assert np.abs(g4["grid"] - expect).max() < 1e-5 * np.abs(expect).max()   # tables are rounded to complex64
+
+
+def _model_image(n, sources):
+    img = np.zeros((n, n), np.complex128)
+    for px, py, amp in sources:
+        img[n // 2 + py, n // 2 + px] = amp                    # pixel (N/2, N/2) is l = m = 0; x (l) is the last axis
+    return img
+
+
+def test_P13_image_to_grid_then_degrid_is_the_visibility_equation(oracle_lib):
+    """O7 inverse (`image_to_grid`) pinned against Eq. 2: a model image of point sources, pre-corrected by
+    the taper and inverse-transformed, then degridded (O5) at random uvw, reproduces V = sum I exp[+2 pi i (ul + vm +
+    w (n - 1))] within the method's own approximation error PER VISIBILITY (no averaging over visibilities as in P2):
+    nearest sub-cell lookup moves a visibility by at most du / (2 O) per axis (phase 2 pi du/(2O) (|l| + |m|)), nearest
+    w-plane by at most w_max / (2 (P - 1)) (phase 2 pi dw |n - 1|), plus 3e-3 for the finite support (P2's bound at
+    O = 64).  A dropped n*n, a wrong shift, a wrong sign of the exponent or of the w-term, a transposed image, or a taper
+    applied after the transform is off by order one.  Cases: w = 0 (PSWF tables) and a wide field with w (WPROJ)."""
+    cases = [
+        (base_params(grid_size=64, cell_size_rad=0.05 / 64, oversample=64), 0.05, True,
+         [(5, -7, 1.0), (-9, 3, 0.5), (0, 0, 0.3)]),
+        (base_params(grid_size=64, cell_size_rad=0.2 / 64, oversample=16, n_wplanes=16, w_max=60.0, support_min=19,
+                     support_max=19, kernel_mode=MODE_WPROJ), 0.2, False, [(12, -10, 1.0), (-9, 13, 0.5)]),
+    ]
+    for params, fov, zero_w, sources in cases:
+        n, o = params["grid_size"], params["oversample"]
+        cell = fov / n
+        uvw, _, _, _ = random_vis(params, 300, seed=5, frac=0.3)
+        if zero_w:
+            uvw[:, 2] = 0
+        dw = 0.0 if zero_w else params["w_max"] / (2 * (params["n_wplanes"] - 1))
+        bound = 0.0
+        for px, py, amp in sources:
+            l, m = px * cell, py * cell
+            bound += abs(amp) * (2 * np.pi * (1.0 / fov) / (2 * o) * (abs(l) + abs(m))
+                                 + 2 * np.pi * dw * abs(np.sqrt(1 - l * l - m * m) - 1) + 3e-3)
+        expect = _point_source_vis(uvw, cell, sources)[:, 0].astype(np.complex128)
+        model_grid = oi.image_to_grid(_model_image(n, sources))
+        pred, rec = oracle_degrid(params, uvw, model_grid[None].astype(np.complex64))
+        assert not rec["drop"].any()
+        err = np.abs(pred["vis"][:, 0] - expect).max()
+        assert bound < 0.15 and 0.3 * bound < err < bound, (err, bound)      # the bound is tight, not a loose allowance
+        # sensitivity: the conjugate (wrong exponent sign), the transposed image (l <-> m) and, with w, a flipped w-term
+        assert np.abs(pred["vis"][:, 0] - np.conj(expect)).max() > 5 * bound
+        wrong, _ = oracle_degrid(params, uvw, oi.image_to_grid(_model_image(n, sources).T)[None].astype(np.complex64))
+        assert np.abs(wrong["vis"][:, 0] - expect).max() > 5 * bound
+        if not zero_w:
+            flipped = _point_source_vis(uvw * np.array([1, 1, -1], np.float32), cell, sources)[:, 0]
+            assert np.abs(pred["vis"][:, 0] - flipped).max() > 5 * bound
+
+
+def test_P13_grid_to_image_inverts_image_to_grid_up_to_taper_squared():
+    """grid_to_image(image_to_grid(x), sum_weights = N^2) * psi^2 = x: both directions divide by the taper (A4 corrects
+    the dirty image, A5 pre-corrects the model), and the inverse DFT is unnormalised."""
+    n = 32
+    rng = np.random.default_rng(2)
+    x = np.zeros((2, n, n), np.complex128)
+    x[:, n // 4:3 * n // 4, n // 4:3 * n // 4] = rng.standard_normal((2, n // 2, n // 2)) + 1j * rng.standard_normal((2, n // 2, n // 2))
+    back = oi.grid_to_image(oi.image_to_grid(x), float(n * n)) * oi.taper_image(n) ** 2
+    assert np.abs(back - x).max() < 1e-9 * np.abs(x).max()
+    # a single centred unit pixel transforms to a constant grid of 1 / psi(0)^2 = 1 (DC and scale)
+    one = np.zeros((n, n), np.complex128)
+    one[n // 2, n // 2] = 1.0
+    assert np.allclose(oi.image_to_grid(one), 1.0, atol=1e-12)

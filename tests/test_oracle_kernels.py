@@ -184,3 +184,37 @@ def test_P12_mosaic_flat_beam_equals_pswf():
     ll, mm = np.meshgrid(l1, l1)
     ratio = fs[1][2][0, 0][1:, 1:] / fs[0][2][0, 0][1:, 1:] * ok.airy(np.hypot(ll, mm), 12, 3e9)[1:, 1:] ** 2
     assert np.allclose(ratio, ok.airy(np.hypot(ll - 0.004, mm + 0.002), 12, 3e9)[1:, 1:] ** 2, rtol=1e-9, atol=1e-12)
+
+
+def test_P14_paper_gridding_function_with_airy_beam_and_leakage():
+    """`_paper_gridding_function` (Eq. 6) pinned with an Airy beam and 1 % leakage, where nothing
+    degenerates: per pixel F_g S^-1 is the inverse of a matrix M^S' that (a) has the off-diagonal cells of
+    M^S = S M S^-1 untouched ("from the diagonal elements"), (b) has Eq. 6 applied to each diagonal beam
+    with ITS OWN max|B_p| (a global maximum, or Eq. 6 applied to M instead of M^S, fails), so that
+    |B'_p| >= eps max|B_p| everywhere including the nulls of the Airy pattern."""
+    nk, eps = 48, 0.2
+    l1 = (np.arange(nk) - nk // 2) * 0.12 / nk                     # out to the second null of a 12 m dish at 1 GHz
+    ll, mm = np.meshgrid(l1, l1)
+    e = ok.airy(np.hypot(ll, mm), 12.0, 1.0e9)
+    assert (e < 0).any() and np.abs(e).min() < 2e-3                # sidelobes and a near-null are inside the field
+    jm = ok.jones_matrix([0.01 * np.exp(0.4j), 0.01 * np.exp(2.0j)], 0.6)
+    m_field = (e * e)[None, None] * ok.mueller(jm, jm)[:, :, None, None]
+    fg = ok._paper_gridding_function(m_field, eps)                 # [s][c][y][x]
+    s_mat, s_inv = ok.STOKES, np.linalg.inv(ok.STOKES)
+    ms = np.einsum("sc,cdyz,dt->styz", s_mat, m_field, s_inv)      # M^S per pixel from the pinned helpers (P8)
+    implied = np.linalg.inv(np.einsum("scyz,ct->yzst", fg, s_inv))  # (F_g S^-1)^-1 = M^S' as the oracle built it
+    maxima = [np.abs(ms[p, p]).max() for p in range(4)]
+    assert max(maxima) / min(maxima) > 1.5                         # the four beams differ: a global maximum would show
+    for s in range(4):
+        for t in range(4):
+            if s != t:
+                assert np.allclose(implied[..., s, t], ms[s, t], rtol=1e-9, atol=1e-12)
+    for p in range(4):
+        b = ms[p, p]
+        beta = ((eps / 2.0) * maxima[p]) ** 2
+        want = b / np.abs(b) * (np.abs(b) + beta / np.abs(b))      # Eq. 6 with this beam's own maximum
+        assert np.allclose(implied[..., p, p], want, rtol=1e-9)
+        assert np.abs(implied[..., p, p]).min() >= eps * maxima[p] * (1 - 1e-9)
+    # and the defining identity: F_g S^-1 M^S' = I_4 at every pixel
+    ident = np.einsum("scyz,ct,yztu->yzsu", fg, s_inv, implied)
+    assert np.allclose(ident, np.eye(4)[None, None], atol=1e-9)
