@@ -10,6 +10,8 @@ followed here is DESIGN.md R2-R5/R8 (= SURVEY.md section 8(c) O1, S2-S5, S8):
   kset = a_index * (2P-1) + (sp + P-1)
   S_p = support_min + 2*rint(((support_max-support_min)/2) * p/(P-1));  taps d in [-h_lo, h_hi],
         h_lo = S//2, h_hi = S-1-h_lo;  drop if the footprint leaves the grid.
+  R17 (invalid input): u, v or w not finite, |u * uv_scale| or |v * uv_scale| >= 2^30, or a_index outside
+        [0, n_aplanes)  ->  dropped, with the fixed record gx = gy = 0, ox = oy = -O/2, sp = 0, kset = 0.
 
 Integer outputs: compared BIT-EXACTLY with the CUDA path.
 """
@@ -41,6 +43,12 @@ def index_visibilities(uvw: np.ndarray, a_index: np.ndarray | None, params: dict
     u = uvw[:, 0].astype(np.float64)
     v = uvw[:, 1].astype(np.float64)
     w = uvw[:, 2].astype(np.float64)
+    a = np.zeros(len(u), dtype=np.int64) if a_index is None else np.asarray(a_index, dtype=np.int64)
+    with np.errstate(invalid="ignore"):
+        invalid = ~(np.isfinite(u) & np.isfinite(v) & np.isfinite(w))
+        invalid |= ~(np.abs(u * uv_scale) < 2.0 ** 30) | ~(np.abs(v * uv_scale) < 2.0 ** 30)
+    invalid |= (a < 0) | (a >= int(params["n_aplanes"]))                # R17
+    u, v, w, a = (np.where(invalid, 0, x) for x in (u, v, w, a))
     qx = np.rint(u * uv_scale).astype(np.int64)
     qy = np.rint(v * uv_scale).astype(np.int64)
     half_o = o // 2
@@ -52,13 +60,15 @@ def index_visibilities(uvw: np.ndarray, a_index: np.ndarray | None, params: dict
     gy = iy + n // 2
     p = np.minimum(p_count - 1, np.rint(np.abs(w) * w_scale).astype(np.int64))
     sp = np.where(w < 0, -p, p)
-    a = np.zeros(len(u), dtype=np.int64) if a_index is None else np.asarray(a_index, dtype=np.int64)
     kset = a * (2 * p_count - 1) + (sp + p_count - 1)
     sched = support_schedule(int(params["support_min"]), int(params["support_max"]), p_count)
     support = sched[p]
     h_lo = support // 2
     h_hi = support - 1 - h_lo
-    drop = (gx - h_lo < 0) | (gx + h_hi >= n) | (gy - h_lo < 0) | (gy + h_hi >= n)
+    drop = (gx - h_lo < 0) | (gx + h_hi >= n) | (gy - h_lo < 0) | (gy + h_hi >= n) | invalid
+    zero = np.int64(0)
+    gx, gy, sp, kset = (np.where(invalid, zero, x) for x in (gx, gy, sp, kset))
+    ox, oy = np.where(invalid, -half_o, ox), np.where(invalid, -half_o, oy)
     return dict(gx=gx, gy=gy, ox=ox, oy=oy, sp=sp, a=a, kset=kset, support=support, drop=drop)
 
 

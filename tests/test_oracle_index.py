@@ -97,3 +97,22 @@ def test_bucket_sort_is_stable_and_partitions():
         assert np.all(rec["kset"][seg] == bucket // (nt * nt))
         assert np.all(rec["gy"][seg] // 32 == (bucket // nt) % nt)
         assert np.all(rec["gx"][seg] // 32 == bucket % nt)
+
+
+def test_invalid_input_is_dropped_with_a_fixed_record():
+    """R17: non-finite uvw, positions beyond 2^30 fine cells and out-of-range a_index are dropped (never indexed)."""
+    params = dict(grid_size=64, cell_size_rad=1e-3, n_wplanes=4, w_max=50.0, support_min=5, support_max=9, oversample=4,
+                  n_aplanes=3)
+    uvw = np.array([[1.0, 2.0, 3.0], [np.nan, 0, 0], [0, np.inf, 0], [0, 0, -np.inf], [3e38, 0, 0], [1.0, 2.0, 3.0],
+                    [1.0, 2.0, 3.0], [5.0, -4.0, -20.0]], np.float32)
+    a = np.array([0, 0, 0, 0, 0, 3, -1, 2], np.int32)
+    rec = oidx.index_visibilities(uvw, a, params)
+    assert list(rec["drop"]) == [False, True, True, True, True, True, True, False]
+    bad = slice(1, 7)
+    for name, val in (("gx", 0), ("gy", 0), ("ox", -2), ("oy", -2), ("sp", 0), ("kset", 0)):
+        assert np.all(rec[name][bad] == val), name
+    packed = oidx.pack_records(rec, 4)
+    assert np.all(packed[bad] == np.array([0, 0, 1 << 16, 0]))
+    assert rec["kset"][7] == 2 * 7 + (-1 + 3) and rec["kset"][0] == 0 * 7 + (0 + 3)
+    keys = oidx.bucket_keys(rec, params, tile=32)
+    assert np.all(keys[bad] == oidx.KEY_DROP)
