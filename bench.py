@@ -9,7 +9,8 @@ A "step" is one pass of the whole hot path over the batch: A1 index -> A2 bucket
 `roofline` is for the dominant kernel (gridding, FP32-FMA bound): achieved = 8 flop x nominal complex MACs / its
 CUDA-event duration (warm call, index reused).  `cpu_baseline` = the oracle on a bounded sample of the same workload.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload config2] [--time-stride s]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload configN] [--time-stride s]
+`--workload config5` feeds its 181 M visibilities in chunks of `--chunk-steps` time steps (one call holds < 2^31 hits).
 N > 1 runs N independent replicas (the path does not shard: BASELINE.json north_star "no sharding, no collectives").
 """
 from __future__ import annotations
@@ -28,6 +29,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 FP32_FMA_PER_CLK_SM = 128          # B200_PROFILING.md / SURVEY 8(d): 128 FP32 lanes per SM
+MEASURED_FFMA2_FMA_PER_CLK_SM = 113.3   # profiles/r1_port_probe.md: FFMA2 x16 at 0.565 clk per warp instruction per SM
 N_SM = 148
 
 
@@ -110,12 +112,6 @@ def job_throughput(units_per_rank, world, ms):
     return world * units_per_rank / (ms * 1e-3)
 
 
-def nominal_cmacs(params, rec):
-    """nominal complex MACs of one gridding pass = n_corr * n_pol * sum_k S_k^2 over kept visibilities."""
-    keep = ~rec["drop"]
-    return int(params["n_corr"]) * int(params["n_pol"]) * int(np.sum(rec["support"][keep].astype(np.int64) ** 2))
-
-
 def oracle_tables(params):
     from oracle import kernels as okern
     tabs, _ = okern.make_tables(params)
@@ -155,6 +151,32 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def workload_chunks(name, time_stride, chunk_steps):
+    """The workload as a list of chunks of whole time steps (one chunk unless the workload is fed in pieces: config 5's
+    181 M visibilities exceed the 2^31 hits one call may hold, include/imager.h "Limits per call")."""
+    from synth import make_workload
+    if name != "config5" or chunk_steps <= 0:
+        return [make_workload(name, time_stride=time_stride)]
+    probe = make_workload(name, time_stride=time_stride, time_range=(0, 1))
+    n_time = probe.notes["n_time_all"]
+    return [make_workload(name, time_stride=time_stride, time_range=(t0, t0 + chunk_steps)) for t0 in range(0, n_time, chunk_steps)]
+
+
+def dram_traffic_of_capture(workload, time_stride):
+    """DRAM bytes per launch of the gridding kernel from the committed `ncu --set full` capture -- used only if that
+    capture was taken on the kernel source that is being benchmarked (profiles/r2_traffic.txt carries its SHA-256)."""
+    import hashlib
+    prof = os.path.join(ROOT, "profiles", "r2_traffic.txt")
+    src = os.path.join(ROOT, "paper_2206_15117_b200", "csrc", "gridder_tiled.cu")
+    if not (os.path.exists(prof) and os.path.exists(src)) or workload != "config2" or time_stride != 1:
+        return None, "no capture for this workload"
+    fields = dict(ln.split(None, 1) for ln in open(prof) if ln.strip() and not ln.startswith("#"))
+    digest = hashlib.sha256(open(src, "rb").read()).hexdigest()
+    if fields.get("gridder_tiled_cu_sha256", "").strip() != digest:
+        return None, "stale: the capture in profiles/r2_traffic.txt is of another version of gridder_tiled.cu"
+    return int(fields["grid_kernel_dram_bytes_per_launch"]), "profiles/r2_traffic.txt (ncu --set full, same kernel source)"
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -168,34 +190,34 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
     from paper_2206_15117_b200 import Plan, REUSE_INDEX
-    from synth import make_workload
-    from oracle import index as oidx           # only for the nominal MAC count (integer bookkeeping) and cpu_baseline
 
-    wl = make_workload(args.workload, time_stride=args.time_stride)
-    params, nvis = wl.params, wl.nvis
+    wls = workload_chunks(args.workload, args.time_stride, args.chunk_steps)
+    params = wls[0].params
+    nvis = sum(w.nvis for w in wls)
+    multi = len(wls) > 1
     n, nc, npol = params["grid_size"], params["n_corr"], params["n_pol"]
-    plan = Plan(params, nvis)                   # the library generates its own kernel tables (A0, untimed)
-    rec = oidx.index_visibilities(wl.uvw, wl.a_index, params)
-    cmacs = nominal_cmacs(params, rec)
-    del rec
+    plan = Plan(params, max(w.nvis for w in wls))      # the library generates its own kernel tables (A0, untimed)
 
-    # resident inputs
-    uvw = torch.from_numpy(wl.uvw).to(dev)
-    vis = torch.from_numpy(wl.vis).to(dev)
-    wts = torch.from_numpy(wl.weights).to(dev)
-    aidx = torch.from_numpy(wl.a_index).to(dev) if wl.a_index is not None else None
+    # resident inputs, chunk by chunk
+    def to_dev(w):
+        return dict(uvw=torch.from_numpy(w.uvw).to(dev), vis=torch.from_numpy(w.vis).to(dev), wts=torch.from_numpy(w.weights).to(dev),
+                    a=torch.from_numpy(w.a_index).to(dev) if w.a_index is not None else None,
+                    out=torch.empty((w.nvis, nc), dtype=torch.complex64, device=dev))
+    data = [to_dev(w) for w in wls]
     grid = torch.zeros((npol, n, n), dtype=torch.complex64, device=dev)
-    vout = torch.empty((nvis, nc), dtype=torch.complex64, device=dev)
     stream = torch.cuda.current_stream()
     launches = 0
+    reuse_degrid = 0 if multi else REUSE_INDEX          # one plan: with several chunks the degridding pass re-indexes too
 
     def step():
         nonlocal launches
         grid.zero_()
-        plan.grid(uvw, vis, wts, grid, aidx)                      # cold: A1 + A2 + A3
-        launches += plan.last_launch_count()
-        plan.degrid(uvw, grid, vout, aidx, flags=REUSE_INDEX)     # A6
-        launches += plan.last_launch_count()
+        for d in data:
+            plan.grid(d["uvw"], d["vis"], d["wts"], grid, d["a"])                 # cold: A1 + A2 + A3
+            launches += plan.last_launch_count()
+        for d in data:
+            plan.degrid(d["uvw"], grid, d["out"], d["a"], flags=reuse_degrid)      # A6 (+ A1 + A2 when chunked)
+            launches += plan.last_launch_count()
 
     def barrier():
         torch.cuda.synchronize()
@@ -223,75 +245,112 @@ def run_ours(args):
     barrier()
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = float(sum(step_ms))
-    # dominant kernel: warm gridding and warm degridding calls timed on their own (index reused)
-    kern = {}
-    for name, fn in (("grid", lambda: plan.grid(uvw, vis, wts, grid, aidx, flags=REUSE_INDEX)),
-                     ("degrid", lambda: plan.degrid(uvw, grid, vout, aidx, flags=REUSE_INDEX))):
-        for _ in range(3):
-            fn()
-        torch.cuda.synchronize()
-        es = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-        for a, b in es:
-            a.record(stream)
-            fn()
-            b.record(stream)
-        torch.cuda.synchronize()
-        kern[name] = float(np.mean([a.elapsed_time(b) for a, b in es]))
+    # dominant kernels: warm gridding and warm degridding calls timed on their own (index reused), summed over the chunks;
+    # the MAC counts come from the plan (imager_index_stats), not from the checker
+    kern = {"grid": 0.0, "degrid": 0.0}
+    stats = {"nominal_cmacs": 0, "executed_cmacs": 0, "n_merged": 0, "n_hits": 0, "n_kept": 0, "n_dropped": 0}
+    reps = args.steps if not multi else min(args.steps, 3)
+    for d in data:
+        if multi:
+            plan.index(d["uvw"], d["a"])
+        st = plan.index_stats()
+        for k in stats:
+            stats[k] += st[k]
+        for name, fn in (("grid", lambda: plan.grid(d["uvw"], d["vis"], d["wts"], grid, d["a"], flags=REUSE_INDEX)),
+                         ("degrid", lambda: plan.degrid(d["uvw"], grid, d["out"], d["a"], flags=REUSE_INDEX))):
+            for _ in range(3 if not multi else 1):
+                fn()
+            torch.cuda.synchronize()
+            es = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+            for a, b in es:
+                a.record(stream)
+                fn()
+                b.record(stream)
+            torch.cuda.synchronize()
+            kern[name] += float(np.mean([a.elapsed_time(b) for a, b in es]))
     barrier()
     sampler.t_end = time.perf_counter()
     sampler.stop_flag = True
+    cmacs, cmacs_exec = stats["nominal_cmacs"], stats["executed_cmacs"]
 
     # end to end: pinned host buffers, H2D of the step's inputs and D2H of its results inside the timed region
-    h_uvw = torch.from_numpy(wl.uvw).pin_memory()
-    h_vis = torch.from_numpy(wl.vis).pin_memory()
-    h_wts = torch.from_numpy(wl.weights).pin_memory()
-    h_a = torch.from_numpy(wl.a_index).pin_memory() if wl.a_index is not None else None
-    h_out = torch.empty((nvis, nc), dtype=torch.complex64).pin_memory()
+    def pin(w):
+        return dict(uvw=torch.from_numpy(w.uvw).pin_memory(), vis=torch.from_numpy(w.vis).pin_memory(),
+                    wts=torch.from_numpy(w.weights).pin_memory(),
+                    a=torch.from_numpy(w.a_index).pin_memory() if w.a_index is not None else None,
+                    out=torch.empty((w.nvis, nc), dtype=torch.complex64).pin_memory())
     h_grid = torch.empty((npol, n, n), dtype=torch.complex64).pin_memory()
-
-    # The call sequence a user with host buffers makes: the visibilities are cut into `e2e_chunks` chunks (gridding is
-    # linear in them), each with its own plan; all H2D copies are queued on a copy stream, chunk k is indexed (imager_index)
-    # as soon as its uvw have arrived and gridded (REUSE_INDEX) as soon as its visibilities and weights have; the grid goes
-    # back to the host while the chunks are degridded, and every chunk's predictions follow it on a third stream.
-    nch = max(1, args.e2e_chunks)
-    bounds = [(k * nvis) // nch for k in range(nch + 1)]
-    chunk_plans = [Plan(params, bounds[k + 1] - bounds[k]) for k in range(nch)] if nch > 1 else [plan]
     h2d_stream, d2h_stream = torch.cuda.Stream(), torch.cuda.Stream()
+    chunk_plans = []
+    if multi:
+        host = [pin(w) for w in wls]
 
-    def e2e_step():
-        h2d_stream.wait_event(stream.record_event())                 # the device buffers are free again
-        ev_u, ev_v = [], []
-        with torch.cuda.stream(h2d_stream):
+        def e2e_step():
+            # chunked workload: per chunk H2D -> imager_grid (cold); D2H grid; per chunk imager_degrid (cold) -> D2H
+            grid.zero_()
+            for d, h in zip(data, host):
+                for k in ("uvw", "vis", "wts", "a"):
+                    if h[k] is not None:
+                        d[k].copy_(h[k], non_blocking=True)
+                plan.grid(d["uvw"], d["vis"], d["wts"], grid, d["a"])
+            h_grid.copy_(grid, non_blocking=True)
+            for d, h in zip(data, host):
+                plan.degrid(d["uvw"], grid, d["out"], d["a"])
+                h["out"].copy_(d["out"], non_blocking=True)
+        e2e_desc = f"{len(wls)} chunks in sequence: H2D chunk -> imager_grid; D2H grid; imager_degrid chunk -> D2H vis"
+        h2d = sum(h[k].numel() * h[k].element_size() for h in host for k in ("uvw", "vis", "wts", "a") if h[k] is not None)
+        d2h = sum(h["out"].numel() * 8 for h in host) + h_grid.numel() * 8
+    else:
+        # The call sequence a user with host buffers makes: the visibilities are cut into `e2e_chunks` chunks (gridding is
+        # linear in them), each with its own plan; all H2D copies are queued on a copy stream, chunk k is indexed
+        # (imager_index) as soon as its uvw have arrived and gridded (REUSE_INDEX) as soon as its visibilities and weights
+        # have; the grid goes back to the host while the chunks are degridded, and every chunk's predictions follow it.
+        w, d = wls[0], data[0]
+        uvw, vis, wts, aidx, vout = d["uvw"], d["vis"], d["wts"], d["a"], d["out"]
+        h = pin(w)
+        h_uvw, h_vis, h_wts, h_a, h_out = h["uvw"], h["vis"], h["wts"], h["a"], h["out"]
+        nch = max(1, args.e2e_chunks)
+        bounds = [(k * nvis) // nch for k in range(nch + 1)]
+        chunk_plans = [Plan(params, bounds[k + 1] - bounds[k]) for k in range(nch)] if nch > 1 else [plan]
+
+        def e2e_step():
+            h2d_stream.wait_event(stream.record_event())                 # the device buffers are free again
+            ev_u, ev_v = [], []
+            with torch.cuda.stream(h2d_stream):
+                for k in range(nch):
+                    sl = slice(bounds[k], bounds[k + 1])
+                    uvw[sl].copy_(h_uvw[sl], non_blocking=True)
+                    if h_a is not None:
+                        aidx[sl].copy_(h_a[sl], non_blocking=True)
+                    ev_u.append(h2d_stream.record_event())
+                    vis[sl].copy_(h_vis[sl], non_blocking=True)
+                    wts[sl].copy_(h_wts[sl], non_blocking=True)
+                    ev_v.append(h2d_stream.record_event())
+            grid.zero_()
             for k in range(nch):
                 sl = slice(bounds[k], bounds[k + 1])
-                uvw[sl].copy_(h_uvw[sl], non_blocking=True)
-                if h_a is not None:
-                    aidx[sl].copy_(h_a[sl], non_blocking=True)
-                ev_u.append(h2d_stream.record_event())
-                vis[sl].copy_(h_vis[sl], non_blocking=True)
-                wts[sl].copy_(h_wts[sl], non_blocking=True)
-                ev_v.append(h2d_stream.record_event())
-        grid.zero_()
-        for k in range(nch):
-            sl = slice(bounds[k], bounds[k + 1])
-            a_k = aidx[sl] if aidx is not None else None
-            stream.wait_event(ev_u[k])
-            chunk_plans[k].index(uvw[sl], a_k)                                               # A1 + A2
-            stream.wait_event(ev_v[k])
-            chunk_plans[k].grid(uvw[sl], vis[sl], wts[sl], grid, a_k, flags=REUSE_INDEX)     # A3
-        d2h_stream.wait_event(stream.record_event())
-        with torch.cuda.stream(d2h_stream):
-            h_grid.copy_(grid, non_blocking=True)
-        for k in range(nch):
-            sl = slice(bounds[k], bounds[k + 1])
-            a_k = aidx[sl] if aidx is not None else None
-            chunk_plans[k].degrid(uvw[sl], grid, vout[sl], a_k, flags=REUSE_INDEX)           # A6
+                a_k = aidx[sl] if aidx is not None else None
+                stream.wait_event(ev_u[k])
+                chunk_plans[k].index(uvw[sl], a_k)                                               # A1 + A2
+                stream.wait_event(ev_v[k])
+                chunk_plans[k].grid(uvw[sl], vis[sl], wts[sl], grid, a_k, flags=REUSE_INDEX)     # A3
             d2h_stream.wait_event(stream.record_event())
             with torch.cuda.stream(d2h_stream):
-                h_out[sl].copy_(vout[sl], non_blocking=True)
-        stream.wait_event(d2h_stream.record_event())
+                h_grid.copy_(grid, non_blocking=True)
+            for k in range(nch):
+                sl = slice(bounds[k], bounds[k + 1])
+                a_k = aidx[sl] if aidx is not None else None
+                chunk_plans[k].degrid(uvw[sl], grid, vout[sl], a_k, flags=REUSE_INDEX)           # A6
+                d2h_stream.wait_event(stream.record_event())
+                with torch.cuda.stream(d2h_stream):
+                    h_out[sl].copy_(vout[sl], non_blocking=True)
+            stream.wait_event(d2h_stream.record_event())
+        e2e_desc = (f"{nch} chunks: H2D uvw_k -> imager_index_k || H2D vis_k, weights_k -> imager_grid_k; "
+                    f"D2H grid || imager_degrid_k -> D2H vis_k")
+        h2d = h_uvw.numel() * 4 + h_vis.numel() * 8 + h_wts.numel() * 4 + (h_a.numel() * 4 if h_a is not None else 0)
+        d2h = h_out.numel() * 8 + h_grid.numel() * 8
 
-    e2e_steps = max(1, min(args.steps, 20))
+    e2e_steps = max(1, min(args.steps, 20 if not multi else 2))
     e2e_step()
     barrier()
     t0 = torch.cuda.Event(enable_timing=True)
@@ -302,8 +361,6 @@ def run_ours(args):
     t1.record(stream)
     barrier()
     e2e_ms = t0.elapsed_time(t1) / e2e_steps
-    h2d = h_uvw.numel() * 4 + h_vis.numel() * 8 + h_wts.numel() * 4 + (h_a.numel() * 4 if h_a is not None else 0)
-    d2h = h_out.numel() * 8 + h_grid.numel() * 8
 
     total_ms, e2e_ms = reduce_times_max([total_ms, e2e_ms], dev)
     if rank != 0:
@@ -313,37 +370,49 @@ def run_ours(args):
     peaks, peaks_kind = load_peaks()
     ms_per_step = total_ms / args.steps
     value = job_throughput(nvis, world, ms_per_step)
-    peak_tflops = N_SM * FP32_FMA_PER_CLK_SM * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 * 2 / 1e12
+    sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
+    peak_tflops = N_SM * FP32_FMA_PER_CLK_SM * sm_mhz * 1e6 * 2 / 1e12
+    peak_measured = N_SM * MEASURED_FFMA2_FMA_PER_CLK_SM * sm_mhz * 1e6 * 2 / 1e12
     achieved = 8.0 * cmacs / (kern["grid"] * 1e-3) / 1e12
-    traffic = None                                  # DRAM bytes per launch of the gridding kernel, from the committed ncu capture
-    prof = os.path.join(ROOT, "profiles", "r1b_traffic.txt")
-    if os.path.exists(prof) and args.workload == "config2" and args.time_stride == 1:
-        for ln in open(prof):
-            if ln.startswith("grid_kernel_dram_bytes_per_launch"):
-                traffic = int(ln.split()[1])
+    traffic, traffic_src = dram_traffic_of_capture(args.workload, args.time_stride)
+    in_bytes = nvis * (12 + 8 * nc + 4 * nc + (4 if wls[0].a_index is not None else 0))
+    grid_bytes = npol * n * n * 8
+    step_desc = ("imager_grid (index+sort+plan+grid) + imager_degrid (index reused)" if not multi else
+                 f"{len(wls)} chunks of {args.chunk_steps} time steps through ONE plan: imager_grid per chunk (index+sort+plan+grid), "
+                 f"then imager_degrid per chunk (index+sort+plan+degrid: the index of another chunk cannot be reused)")
     line = {
         "metric": "visibilities gridded+degridded/sec", "value": value, "unit": "vis/s", "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": args.workload, "nvis": nvis, "grid": n, "n_wplanes": params["n_wplanes"],
                    "support": [params["support_min"], params["support_max"]], "oversample": params["oversample"],
-                   "n_corr": nc, "time_stride": args.time_stride, "parallelism": f"replicas x{world}",
-                   "l2": "inputs (290 MB of visibilities + 33.5 MB grid) exceed the 126 MB L2; no explicit flush",
-                   "step": "imager_grid (index+sort+grid) + imager_degrid (index reused)",
-                   "e2e_step": f"{nch} chunks: H2D uvw_k -> imager_index_k || H2D vis_k, weights_k -> imager_grid_k; D2H grid || imager_degrid_k -> D2H vis_k"},
+                   "n_corr": nc, "time_stride": args.time_stride, "chunks": len(wls), "parallelism": f"replicas x{world}",
+                   "l2": f"inputs ({in_bytes / 1e6:.0f} MB of visibilities + {grid_bytes / 1e6:.1f} MB grid) "
+                         f"{'exceed' if in_bytes + grid_bytes > 126e6 else 'FIT IN'} the 126 MB L2; no explicit flush",
+                   "step": step_desc, "e2e_step": e2e_desc},
         "clocks": sampler.summary(),
         "e2e": {"value": job_throughput(nvis, world, e2e_ms), "unit": "vis/s", "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms},
         "gpu_launches": launches,
         "roofline": {"bound": "alu", "kernel": "gridding (imager_grid, index reused)", "achieved": achieved,
                      "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": traffic,
-                     "peak_kind": f"148 SM x 128 FP32 lanes x 2 flop x {peaks.get('sm_max_mhz', 1965.0):.0f} MHz "
-                                  f"({peaks_kind} max SM clock)",
-                     "kernel_ms": kern["grid"], "nominal_cmacs": cmacs,
+                     "traffic_source": traffic_src,
+                     "peak_kind": f"148 SM x 128 FP32 lanes x 2 flop x {sm_mhz:.0f} MHz ({peaks_kind} max SM clock)",
+                     "frac_of_measured_fma": achieved / peak_measured,
+                     "measured_fma_peak": peak_measured,
+                     "measured_fma_peak_kind": f"148 SM x {MEASURED_FFMA2_FMA_PER_CLK_SM} FMA/clk/SM (FFMA2 issue rate measured on "
+                                               f"this pool's B200: 0.565 clk per warp instruction per SM, profiles/r1_port_probe.md) x 2 flop x {sm_mhz:.0f} MHz",
+                     "kernel_ms": kern["grid"], "nominal_cmacs": cmacs, "executed_cmacs": cmacs_exec,
+                     "note": "achieved / frac count NOMINAL complex MACs (8 flop each: the algorithmic work of the pass); the kernel "
+                             "executes `executed_cmacs` (duplicate visibilities are pre-summed: exact algebra), frac_executed counts those",
+                     "frac_executed": 8.0 * cmacs_exec / (kern["grid"] * 1e-3) / 1e12 / peak_tflops,
+                     "merged_duplicates": stats["n_merged"], "hits": stats["n_hits"],
                      "grid_vis_per_s": nvis / (kern["grid"] * 1e-3), "grid_cmac_per_s": cmacs / (kern["grid"] * 1e-3),
                      "degrid_ms": kern["degrid"], "degrid_vis_per_s": nvis / (kern["degrid"] * 1e-3),
+                     "degrid_cmac_per_s": cmacs / (kern["degrid"] * 1e-3),
                      "degrid_frac": 8.0 * cmacs / (kern["degrid"] * 1e-3) / 1e12 / peak_tflops,
-                     "hbm_gbs_grid": (nvis * (16 + 4 + 8 * nc + 4 * nc) + 2 * npol * n * n * 8) / (kern["grid"] * 1e-3) / 1e9},
+                     "cold_path_ms": ms_per_step - kern["grid"] - kern["degrid"],
+                     "hbm_gbs_grid": (nvis * (16 + 4 + 8 * nc + 4 * nc) + 2 * grid_bytes) / (kern["grid"] * 1e-3) / 1e9},
         "step_ms_all": step_ms,
     }
     if not args.no_cpu_baseline:
@@ -386,6 +455,7 @@ def main():
     ap.add_argument("--time-stride", type=int, default=1, help="keep every n-th time step (1 = the full workload)")
     ap.add_argument("--ref-time-stride", type=int, default=20, help="time-step stride of the CPU oracle's sample")
     ap.add_argument("--e2e-chunks", type=int, default=2, help="chunks of the end-to-end pipeline (1 = one call per stage)")
+    ap.add_argument("--chunk-steps", type=int, default=100, help="config5: time steps per chunk fed through the API")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.steps is None:

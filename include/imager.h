@@ -13,8 +13,18 @@
  * General rules
  *   - Every pointer argument says "dev" (CUDA device memory, caller-owned, e.g. a torch tensor) or "host".
  *   - The library never allocates or frees caller memory.  All device work is enqueued on the given
- *     cuda_stream (a cudaStream_t passed as void*; NULL = the legacy default stream).  The hot calls
- *     (imager_grid / imager_degrid) never synchronise the device; plan creation and the debug exports do.
+ *     cuda_stream (a cudaStream_t passed as void*; NULL = the legacy default stream).
+ *   - Synchronisation contract.  imager_grid / imager_degrid with IMAGER_REUSE_INDEX (the steady state of a major-cycle
+ *     loop) only enqueue work: no host wait, no allocation.  A call that (re)indexes -- imager_index, or the first
+ *     imager_grid / imager_degrid after new (uvw, a_index) -- waits ONCE for cuda_stream (cudaStreamSynchronize: the
+ *     sizes of the hit lists are read back to bound the launches that follow and to guard their 32-bit offsets) and may
+ *     grow plan-owned scratch if the data need more than the estimate made at the first call.  Never a device-wide
+ *     synchronisation.  Plan creation and the debug / statistics exports synchronise.
+ *   - A plan is bound to ONE stream at a time: its work queues and cached hit lists are plan state, so calls on the
+ *     same plan must be issued on the same stream (or be ordered by the caller); use one plan per concurrent stream.
+ *   - Limits per call: nvis <= max_nvis, and fewer than 2^31 hits (visibility x 16 x 32-cell strip pairs; about 4 per
+ *     visibility at support 15, 15 at support 63) -- IMAGER_ERR_TOO_MANY_VIS otherwise.  Larger data sets are fed in
+ *     chunks: gridding accumulates into the caller's grid, degridding is per visibility.
  *   - Every call returns 0 on success or a negative imager_status.  No exceptions, no abort, no printing.
  *     imager_last_error() gives a thread-local message for the last failure on this thread.
  *     Asynchronous CUDA faults surface on the next call or at the caller's synchronisation.
@@ -104,11 +114,13 @@ int imager_plan_create(const imager_params* params, void* cuda_stream, imager_pl
 /* Steps A1 + A2 on their own: index and bucket (uvw, a_index) and plan the work lists of the gridding / degridding
  * kernels, so that later imager_grid / imager_degrid calls with IMAGER_REUSE_INDEX start at once (e.g. while the
  * visibilities are still being copied to the device).  uvw dev float32 [nvis][3], a_index dev int32 [nvis] or NULL.
- * Synchronises the stream once (the list sizes are read back).  Errors: INVALID_ARG, TOO_MANY_VIS, NOMEM, CUDA. */
+ * Synchronises the stream once (the list sizes are read back).  Errors: INVALID_ARG, TOO_MANY_VIS (nvis > max_nvis or
+ * 2^31 hits or more), NOMEM, CUDA. */
 int imager_index(imager_plan* plan, int64_t nvis, const float* uvw, const int32_t* a_index, void* cuda_stream);
 
 /* Gridding.  Accumulates into `grid` (the caller zeroes it); visibilities whose footprint leaves the
- * grid are skipped and counted (R8).  uvw dev float32 [nvis][3] in wavelengths ("baseline vectors ... in
+ * grid are skipped and counted (R8), and so are invalid ones (R17: u, v or w not finite or beyond 2^30 fine cells,
+ * a_index outside [0, n_aplanes)): nothing is ever indexed from them.  uvw dev float32 [nvis][3] in wavelengths ("baseline vectors ... in
  * units of wavelength"); vis dev complex64 [nvis][n_corr]; weights dev float32 [nvis][n_corr]; a_index dev
  * int32 [nvis] in [0, n_aplanes) or NULL (= 0); grid dev complex64 [n_pol][N][N]; sum_weights dev double
  * [n_corr] or NULL, accumulated with the weights of the kept visibilities.
@@ -127,7 +139,9 @@ int imager_plan_destroy(imager_plan* plan);
 
 /* ---- surrounding stages, built but outside the timed hot path (BASELINE.json north_star item 3) ---- */
 
-/* direction = +1: grid -> image: centred forward DFT (cuFFT) of each [N][N] plane in place, then divide by
+/* (The survey's proposed `imager_taper_correct` lives inside this call: the division by psi psi is fused with the
+ * centring sign flips around the cuFFT transform.)
+ * direction = +1: grid -> image: centred forward DFT (cuFFT) of each [N][N] plane in place, then divide by
  * psi(l) psi(m) and by norm (pass the sum of weights; 0 means 1).  direction = -1: image -> grid: divide by
  * psi psi, then the centred unnormalised inverse DFT (R1: signs follow Eq. 2).  data dev complex64. */
 int imager_grid_image_transform(imager_plan* plan, float* data, int32_t direction, double norm, void* cuda_stream);
@@ -154,8 +168,19 @@ int imager_debug_index(imager_plan* plan, int64_t nvis, const float* uvw, const 
 int imager_debug_kernels(imager_plan* plan, int32_t kset, int32_t which, float* host_out, int32_t* support_out);
 
 /* info: [0] n_sets, [1] bucket tile size, [2] n_buckets, [3] key bits, [4] dropped visibilities of the last
- * indexing (synchronises), [5] GPU kernel launches issued by the last imager_grid / imager_degrid call. */
+ * indexing, [5] GPU kernel launches issued by the last imager_grid / imager_degrid call, [6] complex elements of one
+ * table set collection, [7] kept visibilities of the last indexing.  [4] and [7] are read with a blocking copy on the
+ * legacy default stream (it waits for work on that stream and on blocking streams, not for the whole device). */
 int imager_plan_info(imager_plan* plan, int64_t info_out[8]);
+
+/* Statistics of the current index (built by the last imager_index / imager_grid / imager_degrid / imager_debug_index
+ * call); synchronises cuda_stream.  out[0] kept visibilities, [1] dropped ones, [2] duplicates merged into another
+ * visibility of the same (kernel set, cell, sub-cell) (pre-summed: exact algebra, R16), [3] nominal complex
+ * multiply-accumulates of one gridding (= one degridding) pass, n_corr n_pol sum over kept visibilities of S^2,
+ * [4] the complex multiply-accumulates the tiled kernels execute (merged duplicates excluded), [5] hits (visibility x
+ * 16 x 32 strip pairs) and [6] work items of the tiled plan (0 before it is built), [7] 0.
+ * Errors: INVALID_ARG (NULL, no index yet), CUDA. */
+int imager_index_stats(imager_plan* plan, int64_t out[8], void* cuda_stream);
 
 /* Number of GPU kernels the last imager_grid / imager_degrid / imager_debug_index call on this plan launched
  * (host-side counter, no synchronisation); negative status on a NULL plan. */

@@ -22,6 +22,7 @@ DEGRID_RESIDUAL = 16
 
 EXPORTS = ("imager_plan_create", "imager_index", "imager_grid", "imager_degrid", "imager_plan_destroy",
            "imager_grid_image_transform", "imager_mosaic_correct", "imager_debug_index", "imager_debug_kernels", "imager_plan_info",
+           "imager_index_stats",
            "imager_last_launch_count", "imager_last_error")
 
 
@@ -62,6 +63,7 @@ def load_library() -> ctypes.CDLL:
                                        POINTER(c_int64), c_void_p]
     lib.imager_debug_kernels.argtypes = [c_void_p, c_int32, c_int32, c_void_p, POINTER(c_int32)]
     lib.imager_plan_info.argtypes = [c_void_p, POINTER(c_int64)]
+    lib.imager_index_stats.argtypes = [c_void_p, POINTER(c_int64), c_void_p]
     lib.imager_last_launch_count.argtypes = [c_void_p]
     _lib = lib
     return lib
@@ -194,6 +196,12 @@ class Plan:
         out = (c_int64 * 8)()
         _check(load_library().imager_plan_info(self._h, out), "imager_plan_info")
         names = ("n_sets", "bucket_tile", "n_buckets", "key_bits", "n_dropped", "last_launches", "table_elems", "n_kept")
+        return dict(zip(names, [int(x) for x in out]))
+
+    def index_stats(self, stream=None) -> dict:
+        out = (c_int64 * 8)()
+        _check(load_library().imager_index_stats(self._h, out, _stream_ptr(stream)), "imager_index_stats")
+        names = ("n_kept", "n_dropped", "n_merged", "nominal_cmacs", "executed_cmacs", "n_hits", "n_items")
         return dict(zip(names, [int(x) for x in out]))
 
     def debug_index(self, uvw, a_index=None, stream=None) -> dict:

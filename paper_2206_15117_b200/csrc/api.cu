@@ -127,9 +127,10 @@ extern "C" int imager_plan_create(const imager_params* params, void* cuda_stream
         return IMAGER_ERR_UNSUPPORTED;
     }
     pl->n_buckets = (int)nb;
+    pl->key_drop = (uint32_t)(nb * O * O);                // one more than the largest valid key
     pl->key_bits = 1;
-    while (((int64_t)1 << pl->key_bits) < nb * O * O) pl->key_bits++;
-    pl->sort_passes = 4;                                  // the drop key has all 32 bits set
+    while (((int64_t)1 << pl->key_bits) <= nb * O * O) pl->key_bits++;      // bits of the drop key
+    pl->sort_passes = (pl->key_bits + 7) / 8;
     const int64_t mv = p.max_nvis > 0 ? p.max_nvis : 1;
     const int64_t n_chunks = (mv + kSortChunk - 1) / kSortChunk;
     const int64_t hist_len = 256 * n_chunks;
@@ -245,7 +246,10 @@ extern "C" int imager_debug_index(imager_plan* plan, int64_t nvis, const float* 
     const int b = plan->sorted_buf;
     if (records_out && nvis) IMAGER_CUDA(cudaMemcpy(records_out, plan->d_rec, nvis * sizeof(imager_record), cudaMemcpyDeviceToHost));
     if (perm_out && nvis) IMAGER_CUDA(cudaMemcpy(perm_out, plan->d_perm[b], nvis * sizeof(int32_t), cudaMemcpyDeviceToHost));
-    if (keys_out && nvis) IMAGER_CUDA(cudaMemcpy(keys_out, plan->d_key[b], nvis * sizeof(uint32_t), cudaMemcpyDeviceToHost));
+    if (keys_out && nvis) {
+        IMAGER_CUDA(cudaMemcpy(keys_out, plan->d_key[b], nvis * sizeof(uint32_t), cudaMemcpyDeviceToHost));
+        for (int64_t i = nvis - 1; i >= 0 && keys_out[i] == plan->key_drop; --i) keys_out[i] = kKeyDrop;   // sorted: drops last
+    }
     if (bucket_offset_out)
         IMAGER_CUDA(cudaMemcpy(bucket_offset_out, plan->d_bucket_offset, ((size_t)plan->n_buckets + 1) * sizeof(int32_t), cudaMemcpyDeviceToHost));
     if (n_kept_out) {
@@ -268,6 +272,13 @@ extern "C" int imager_debug_kernels(imager_plan* plan, int32_t kset, int32_t whi
     return 0;
 }
 
+extern "C" int imager_index_stats(imager_plan* plan, int64_t out[8], void* cuda_stream) {
+    g_err[0] = 0;
+    if (!plan || !out) { set_error("NULL argument"); return IMAGER_ERR_INVALID_ARG; }
+    if (!plan->index_valid) { set_error("no index yet: call imager_index / imager_grid / imager_degrid first"); return IMAGER_ERR_INVALID_ARG; }
+    return tiled_index_stats(plan, out, (cudaStream_t)cuda_stream);
+}
+
 extern "C" int imager_last_launch_count(imager_plan* plan) {
     return plan ? plan->last_launches : (int)IMAGER_ERR_INVALID_ARG;
 }
@@ -276,8 +287,7 @@ extern "C" int imager_plan_info(imager_plan* plan, int64_t info_out[8]) {
     g_err[0] = 0;
     if (!plan || !info_out) { set_error("NULL argument"); return IMAGER_ERR_INVALID_ARG; }
     int32_t c[2] = {0, 0};
-    IMAGER_CUDA(cudaDeviceSynchronize());
-    IMAGER_CUDA(cudaMemcpy(c, plan->d_counters, sizeof(c), cudaMemcpyDeviceToHost));
+    IMAGER_CUDA(cudaMemcpy(c, plan->d_counters, sizeof(c), cudaMemcpyDeviceToHost));     // blocking copy on the legacy stream
     info_out[0] = plan->n_sets;
     info_out[1] = kBucketTile;
     info_out[2] = plan->n_buckets;

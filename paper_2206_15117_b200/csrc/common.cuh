@@ -10,7 +10,7 @@
 namespace imager {
 
 constexpr int kBucketTile = 32;          // bucketing tile (cells); DESIGN.md "Bucketing key"
-constexpr uint32_t kKeyDrop = 0xFFFFFFFFu;
+constexpr uint32_t kKeyDrop = 0xFFFFFFFFu;   // exported key of a dropped visibility (the oracle's KEY_DROP)
 constexpr int kSortChunk = 2048;         // items per warp in the radix sort
 constexpr int kNumSMs = 148;             // B200
 
@@ -28,6 +28,7 @@ int cuda_fail(cudaError_t e, const char* what);
 struct imager_plan {
     imager_params p;                     // copy of the caller's params (host pointers cleared)
     int n_sets = 0, nt = 0, n_buckets = 0, key_bits = 0, sort_passes = 0;
+    uint32_t key_drop = 0;               // internal sort key of a dropped visibility: n_buckets * O * O
     double uv_scale = 0, w_scale = 0;
     std::vector<int> plane_support;      // S_p, p = 0..P-1
     std::vector<int64_t> set_offset;     // per kernel set, in complex elements (n_sets + 1)
@@ -89,6 +90,7 @@ int launch_grid_tiled(imager_plan* pl, int64_t nvis, const float2* vis, const fl
 int launch_degrid_tiled(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, int residual, cudaStream_t st);
 void tiled_release(imager_plan* pl);
 int tiled_prepare(imager_plan* pl, int64_t nvis, cudaStream_t st);
+int tiled_index_stats(imager_plan* pl, int64_t out[8], cudaStream_t st);
 
 // tables.cu
 int build_tables(imager_plan* pl, const imager_params* user, cudaStream_t st);

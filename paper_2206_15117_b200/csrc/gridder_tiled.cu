@@ -57,8 +57,7 @@ constexpr int kGridStageBytes = (kGridThreads / 32) * kStageSlots * 16;
 constexpr int kMaxSmem = 227 * 1024;
 constexpr int kRedSlots = 8;                           // degridding: hits per transposed reduction
 constexpr int kRedBytes = kWarps * kRedSlots * 32 * 8;
-constexpr int kTableBudget = kMaxSmem - kStageBytes - kRedBytes - 1024;   // stage + degridding reduction buffer + static
-static_assert(kGridStageBytes <= kStageBytes + kRedBytes, "the gridding kernel's staging must fit beside the tables");
+constexpr int kTableBudget = kMaxSmem - (kStageBytes + kRedBytes > kGridStageBytes ? kStageBytes + kRedBytes : kGridStageBytes) - 1024;   // 1 KB: static
 constexpr int64_t kMaxPlanCells = (int64_t)1 << 30;   // (geometry unit, strip) pairs: 12 bytes of planner state each
 constexpr uint32_t kTapBias = 1u << 20;
 
@@ -275,10 +274,12 @@ __device__ __forceinline__ VisHits vis_hits(const PlanArgs& a, const uint2 geo) 
     return v;
 }
 
-__global__ void count_hits_kernel(const PlanArgs a, const int32_t* __restrict__ counters, int32_t* __restrict__ hits) {
+__global__ void count_hits_kernel(const PlanArgs a, const int32_t* __restrict__ counters, int32_t* __restrict__ hits,
+                                  unsigned long long* __restrict__ total) {
     const Geometry& g = a.g;
     const int n_kept = counters[0];
     const int lane = threadIdx.x & 31;
+    int mine = 0;                              // hits of this thread's visibilities (the 64-bit total guards the int32 scan)
     // warp-uniform trip count: the lanes of a warp hold consecutive sorted visibilities, which mostly meet the same strips
     for (int i0 = (blockIdx.x * blockDim.x + threadIdx.x) - lane; i0 < n_kept; i0 += gridDim.x * blockDim.x) {
         const int i = i0 + lane;
@@ -288,6 +289,7 @@ __global__ void count_hits_kernel(const PlanArgs a, const int32_t* __restrict__ 
             const uint2 geo = a.sgeo[i];
             if (!(geo.x & 0x8000u)) v = vis_hits(a, geo);                      // merged duplicates have no hits of their own
         }
+        mine += v.n;
 #if IMAGER_AGGREGATE
         const int n_max = __reduce_max_sync(0xffffffffu, v.n);
         for (int t = 0; t < n_max; ++t) {
@@ -304,6 +306,8 @@ __global__ void count_hits_kernel(const PlanArgs a, const int32_t* __restrict__ 
         }
 #endif
     }
+    mine = __reduce_add_sync(0xffffffffu, mine);       // < 2^31: a thread sees at most 2^31 / gridDim visibilities x 162 strips
+    if (lane == 0 && mine) atomicAdd(total, (unsigned long long)mine);
 }
 
 // items[cell] = ceil(hits[cell] / kItemHits); entry n_cells (the terminator of the exclusive scans) is 0 in both
@@ -339,26 +343,45 @@ __global__ void emit_hits_kernel(const PlanArgs a, const int32_t* __restrict__ c
 #else
         const int n_max = v.n;
 #endif
-        for (int t = 0; t < n_max; ++t) {
-            const bool on = t < v.n;
-            const int ty = on ? t / v.nsx : 0, tx = t - ty * v.nsx;
-            const long long cell = on ? v.cell0 + (int64_t)ty * g.strips_per_row + tx : -1ll - lane;
-            int pos;
+        // four strips at a time: their cursor atomics (which return a value) are in flight together
+        for (int t0 = 0; t0 < n_max; t0 += 4) {
+            long long cell[4];
+            unsigned peers[4];
+            int base[4], start[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int t = t0 + q;
+                const bool on = t < v.n;
+                const int ty = on ? t / v.nsx : 0, tx = t - ty * v.nsx;
+                cell[q] = on ? v.cell0 + (int64_t)ty * g.strips_per_row + tx : -1ll - lane;
+                base[q] = start[q] = 0;
+                peers[q] = 1u << lane;
+                if (t < n_max) {                                            // warp-uniform
 #if IMAGER_AGGREGATE
-            const unsigned peers = __match_any_sync(0xffffffffu, cell);
-            const int leader = __ffs(peers) - 1;
-            int base = 0;
-            if (on && lane == leader) base = atomicAdd(cursor + cell, __popc(peers));
-            base = __shfl_sync(0xffffffffu, base, leader);
-            pos = base + __popc(peers & lt_mask);
+                    peers[q] = __match_any_sync(0xffffffffu, cell[q]);
+                    if (on && lane == __ffs(peers[q]) - 1) base[q] = atomicAdd(cursor + cell[q], __popc(peers[q]));
 #else
-            pos = atomicAdd(cursor + cell, 1);
+                    if (on) base[q] = atomicAdd(cursor + cell[q], 1);
 #endif
-            if (on) {
-                const int dx0 = (v.sx0 + tx) * kStripW - v.x0, dy0 = (v.sy0 + ty) * kStripH - v.y0;   // taps of the strip origin
-                const uint32_t ctrl = hit_ctrl(dx0, dy0, v.S, v.subl, group_slices);
-                const int tapoff = v.subl * slice_taps + (dy0 + kPadY) * pitch + dx0 + kPadX;
-                hit_tmp[(int64_t)hit_start[cell] + pos] = make_uint2((uint32_t)i, (uint32_t)(tapoff + (int)kTapBias) | (ctrl << 24));
+                    if (on) start[q] = hit_start[cell[q]];
+                }
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int t = t0 + q;
+                if (t >= n_max) break;                                      // warp-uniform
+#if IMAGER_AGGREGATE
+                const int pos = __shfl_sync(0xffffffffu, base[q], __ffs(peers[q]) - 1) + __popc(peers[q] & lt_mask);
+#else
+                const int pos = base[q];
+#endif
+                if (t < v.n) {
+                    const int ty = t / v.nsx, tx = t - ty * v.nsx;
+                    const int dx0 = (v.sx0 + tx) * kStripW - v.x0, dy0 = (v.sy0 + ty) * kStripH - v.y0;   // taps of the strip origin
+                    const uint32_t ctrl = hit_ctrl(dx0, dy0, v.S, v.subl, group_slices);
+                    const int tapoff = v.subl * slice_taps + (dy0 + kPadY) * pitch + dx0 + kPadX;
+                    hit_tmp[(int64_t)start[q] + pos] = make_uint2((uint32_t)i, (uint32_t)(tapoff + (int)kTapBias) | (ctrl << 24));
+                }
             }
         }
     }
@@ -736,7 +759,9 @@ grid_tiled_kernel(const TiledArgs a, const float2* __restrict__ sval, float2* __
 // sum conj(t) g over their cells:  P += t * g.x, Q += t * g.y,  conj(t) g = (P.x + Q.y) + i (Q.x - P.y).
 // The 32 partial sums of a hit go to a per-warp shared buffer red[slot][lane]; every 8 hits the buffer is summed
 // by a transposed read (lane = slot + 8 * quarter sums 8 columns, two shuffles join the quarters) and the result is
-// added to the visibility's sorted-order sum with one red.global.add.v2.f32 per hit.
+// added to the visibility's sorted-order sum with one red.global.add.v2.f32 per hit.  (Measured alternative, DESIGN.md
+// section 6.4: the same sum by one mma.sync.m16n8k8 per hit with a TF32 head / tail split takes the reduction off the
+// shared-memory pipe -- 77 % -> 54 % busy -- but the longer bodies miss the instruction cache more: 4.9 ms against 4.1.)
 
 __device__ __forceinline__ void sts64(uint32_t addr, float2 v) {
     asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(v.x), "f"(v.y) : "memory");
@@ -916,14 +941,16 @@ struct TiledState {
     Item* d_item_rec = nullptr;
     Block* d_blocks = nullptr;
     int64_t cap_hits = 0, cap_items = 0, cap_blocks = 0, cap_tmp = 0;
-    int32_t* h_totals = nullptr;          // pinned [2]
+    int64_t* h_totals = nullptr;          // pinned [2]: hits (64-bit count), items
+    unsigned long long* d_total = nullptr;  // 64-bit hit count of count_hits_kernel
+    bool initialised = false;             // set once every allocation of the first prepare() has succeeded
     uint2* d_sgeo = nullptr;
     int32_t* d_rep = nullptr;             // [max_nvis] representative of every sorted visibility (IMAGER_DEDUPE)
     float2* d_sval = nullptr;
     int64_t plan_epoch = -1;
     int32_t blocks_cap = 0;               // the two-ended block queue lives in d_blocks[0 .. blocks_cap)
     Geometry g;
-    int smem_bytes = 0;
+    int smem_bytes = 0;                   // the largest resident table group (the kernels add their staging)
 };
 
 // taps per padded table row: >= S + 2 kPadX and such that the lane block of a half-warp wavefront reads conflict-free
@@ -971,7 +998,7 @@ static TiledState* state_of(imager_plan* pl) {
         sp.gu_base = n_gu;
         n_gu += sp.n_groups;
         for (int q = 0; q < sp.n_groups; ++q) st->gu_set.push_back(k);
-        st->smem_bytes = std::max<int>(st->smem_bytes, (int)(gs * slice_bytes) + kStageBytes);
+        st->smem_bytes = std::max<int>(st->smem_bytes, (int)(gs * slice_bytes));
         st->plan[k] = sp;
     }
     Geometry& g = st->g;
@@ -1004,6 +1031,7 @@ void tiled_release(imager_plan* pl) {
     cudaFree(st->d_sgeo);
     cudaFree(st->d_rep);
     cudaFree(st->d_sval);
+    cudaFree(st->d_total);
     if (st->h_totals) cudaFreeHost(st->h_totals);
     delete st;
     pl->tiled = nullptr;
@@ -1021,35 +1049,64 @@ static int grow(T** ptr, int64_t* cap, int64_t need) {
     return 0;
 }
 
-// (Re)build the hit lists, items and blocks for the current index.  Synchronises the stream once (the sizes of the
-// lists are read back to size their storage); cached until the next re-indexing.
-static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
+// One-time allocations of the tiled path.  The hit lists are pre-sized from max_nvis and the mean number of strips a
+// footprint meets (over the kernel sets), so that in the steady state -- and normally in the first call too -- no hot
+// call allocates; prepare() still grows them if a data set needs more.
+static int init_buffers(imager_plan* pl, TiledState* st, cudaStream_t stream) {
     const int64_t mv = std::max<int64_t>(pl->p.max_nvis, 1);
     const Geometry& g = st->g;
     const int64_t n_cells = (int64_t)g.n_gu * g.n_strips;
-    if (!st->d_plan) {
-        IMAGER_CUDA(cudaMalloc(&st->d_plan, pl->n_sets * sizeof(SetPlan)));
-        IMAGER_CUDA(cudaMalloc(&st->d_gu_set, st->gu_set.size() * sizeof(int32_t)));
-        IMAGER_CUDA(cudaMemcpyAsync(st->d_plan, st->plan.data(), pl->n_sets * sizeof(SetPlan), cudaMemcpyHostToDevice, stream));
-        IMAGER_CUDA(cudaMemcpyAsync(st->d_gu_set, st->gu_set.data(), st->gu_set.size() * sizeof(int32_t),
-                                    cudaMemcpyHostToDevice, stream));
-        int64_t tmp_len = 16;
-        for (int64_t n = n_cells + 1; n > 1; n = (n + 1023) / 1024) tmp_len += (n + 1023) / 1024 + 1;
-        IMAGER_CUDA(cudaMalloc(&st->d_hits, (n_cells + 1) * sizeof(int32_t)));
-        IMAGER_CUDA(cudaMalloc(&st->d_items, (n_cells + 1) * sizeof(int32_t)));
-        IMAGER_CUDA(cudaMalloc(&st->d_cursor, (n_cells + 1) * sizeof(int32_t)));
-        IMAGER_CUDA(cudaMalloc(&st->d_scan_tmp, tmp_len * sizeof(int32_t)));
-        IMAGER_CUDA(cudaMalloc(&st->d_sgeo, mv * sizeof(uint2)));
+    IMAGER_CUDA(cudaMalloc(&st->d_plan, pl->n_sets * sizeof(SetPlan)));
+    IMAGER_CUDA(cudaMalloc(&st->d_gu_set, st->gu_set.size() * sizeof(int32_t)));
+    IMAGER_CUDA(cudaMemcpyAsync(st->d_plan, st->plan.data(), pl->n_sets * sizeof(SetPlan), cudaMemcpyHostToDevice, stream));
+    IMAGER_CUDA(cudaMemcpyAsync(st->d_gu_set, st->gu_set.data(), st->gu_set.size() * sizeof(int32_t),
+                                cudaMemcpyHostToDevice, stream));
+    int64_t tmp_len = 16;
+    for (int64_t n = n_cells + 1; n > 1; n = (n + 1023) / 1024) tmp_len += (n + 1023) / 1024 + 1;
+    IMAGER_CUDA(cudaMalloc(&st->d_hits, (n_cells + 1) * sizeof(int32_t)));
+    IMAGER_CUDA(cudaMalloc(&st->d_items, (n_cells + 1) * sizeof(int32_t)));
+    IMAGER_CUDA(cudaMalloc(&st->d_cursor, (n_cells + 1) * sizeof(int32_t)));
+    IMAGER_CUDA(cudaMalloc(&st->d_scan_tmp, tmp_len * sizeof(int32_t)));
+    IMAGER_CUDA(cudaMalloc(&st->d_sgeo, mv * sizeof(uint2)));
 #if IMAGER_DEDUPE
-        IMAGER_CUDA(cudaMalloc(&st->d_rep, mv * sizeof(int32_t)));
-        IMAGER_CUDA(cudaFuncSetAttribute(sorted_geo_dedupe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kDedupeSmem));
+    IMAGER_CUDA(cudaMalloc(&st->d_rep, mv * sizeof(int32_t)));
+    IMAGER_CUDA(cudaFuncSetAttribute(sorted_geo_dedupe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kDedupeSmem));
 #endif
-        IMAGER_CUDA(cudaMalloc(&st->d_sval, mv * pl->p.n_corr * sizeof(float2)));
-        IMAGER_CUDA(cudaMallocHost(&st->h_totals, 2 * sizeof(int32_t)));
-        IMAGER_CUDA(cudaFuncSetAttribute(grid_tiled_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
-        IMAGER_CUDA(cudaFuncSetAttribute(grid_tiled_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
-        IMAGER_CUDA(cudaFuncSetAttribute(degrid_tiled_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
-        IMAGER_CUDA(cudaFuncSetAttribute(degrid_tiled_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
+    IMAGER_CUDA(cudaMalloc(&st->d_sval, mv * pl->p.n_corr * sizeof(float2)));
+    IMAGER_CUDA(cudaMalloc(&st->d_total, sizeof(unsigned long long)));
+    IMAGER_CUDA(cudaMallocHost(&st->h_totals, 2 * sizeof(int64_t)));
+    IMAGER_CUDA(cudaFuncSetAttribute(grid_tiled_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
+    IMAGER_CUDA(cudaFuncSetAttribute(grid_tiled_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
+    IMAGER_CUDA(cudaFuncSetAttribute(degrid_tiled_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
+    IMAGER_CUDA(cudaFuncSetAttribute(degrid_tiled_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxSmem - 1024));
+    // expected strips per footprint: a footprint of S cells starting anywhere meets (S - 1) / W + 1 strips on average
+    double per_vis = 0.0;
+    for (int k = 0; k < pl->n_sets; ++k) {
+        const double S = pl->set_support[k];
+        per_vis += ((S - 1.0) / kStripW + 1.0) * ((S - 1.0) / kStripH + 1.0);
+    }
+    per_vis /= std::max(pl->n_sets, 1);
+    const int64_t est_hits = std::min<int64_t>((int64_t)(per_vis * 1.25 * (double)mv) + 4096, (int64_t)0x7ffffff0);
+    int rc = grow(&st->d_hit_rec, &st->cap_hits, est_hits);
+    if (!rc) rc = grow(&st->d_hit_tmp, &st->cap_tmp, est_hits);
+    if (!rc) rc = grow(&st->d_item_rec, &st->cap_items, est_hits / kItemHits + n_cells / 8 + 1024);
+    return rc;
+}
+
+// (Re)build the hit lists, items and blocks for the current index.  Synchronises the stream once (the sizes of the
+// lists are read back: they bound the launches that follow and guard the 32-bit offsets); cached until the next
+// re-indexing.  Limit per call: fewer than 2^31 hits (visibility x strip pairs) -- larger data sets are fed in chunks
+// (gridding accumulates into the caller's grid).
+static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
+    const Geometry& g = st->g;
+    const int64_t n_cells = (int64_t)g.n_gu * g.n_strips;
+    if (!st->initialised) {
+        const int rc = init_buffers(pl, st, stream);
+        if (rc) {                                     // start clean at the next call instead of running on half a state
+            tiled_release(pl);
+            return rc;
+        }
+        st->initialised = true;
     }
     if (st->plan_epoch == pl->index_epoch) return 0;
 #if IMAGER_DEDUPE
@@ -1066,20 +1123,24 @@ static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
     pa.set_support = pl->d_set_support;
     pa.sgeo = st->d_sgeo;
     IMAGER_CUDA(cudaMemsetAsync(st->d_hits, 0, (n_cells + 1) * sizeof(int32_t), stream));
-    count_hits_kernel<<<8 * kNumSMs, 256, 0, stream>>>(pa, pl->d_counters, st->d_hits);
+    IMAGER_CUDA(cudaMemsetAsync(st->d_total, 0, sizeof(unsigned long long), stream));
+    count_hits_kernel<<<8 * kNumSMs, 256, 0, stream>>>(pa, pl->d_counters, st->d_hits, st->d_total);
+    IMAGER_CUDA(cudaMemcpyAsync(&st->h_totals[0], st->d_total, sizeof(int64_t), cudaMemcpyDeviceToHost, stream));
     items_from_hits_kernel<<<2 * kNumSMs, 256, 0, stream>>>(n_cells, st->d_hits, st->d_items);
     pl->last_launches += 3;
     int rc = exclusive_scan_i32(pl, st->d_hits, n_cells + 1, st->d_scan_tmp, stream);
     if (rc) return rc;
     rc = exclusive_scan_i32(pl, st->d_items, n_cells + 1, st->d_scan_tmp, stream);
     if (rc) return rc;
-    IMAGER_CUDA(cudaMemcpyAsync(&st->h_totals[0], st->d_hits + n_cells, sizeof(int32_t), cudaMemcpyDeviceToHost, stream));
-    IMAGER_CUDA(cudaMemcpyAsync(&st->h_totals[1], st->d_items + n_cells, sizeof(int32_t), cudaMemcpyDeviceToHost, stream));
+    int32_t* h_items32 = reinterpret_cast<int32_t*>(&st->h_totals[1]);
+    h_items32[1] = 0;
+    IMAGER_CUDA(cudaMemcpyAsync(h_items32, st->d_items + n_cells, sizeof(int32_t), cudaMemcpyDeviceToHost, stream));
     IMAGER_CUDA(cudaStreamSynchronize(stream));
-    const int64_t n_hits = st->h_totals[0], n_items = st->h_totals[1];
-    if (n_hits < 0 || n_items < 0) {
-        set_error("hit lists exceed 2^31 entries");
-        return IMAGER_ERR_UNSUPPORTED;
+    const int64_t n_hits = st->h_totals[0], n_items = h_items32[0];
+    if (n_hits > (int64_t)0x7ffffff0) {              // the 32-bit scan above has wrapped: nothing after this point may use it
+        set_error("%lld hits (visibility x strip pairs) in one call exceed the limit of 2^31: feed the visibilities in chunks",
+                  (long long)n_hits);
+        return IMAGER_ERR_TOO_MANY_VIS;
     }
     const int n_sc = g.n_pol * g.n_corr;
     const int64_t max_blocks = (n_hits / kBlockHits + n_hits / (kTailFrac * (kBlockHits / kTailDiv)) + (int64_t)g.n_gu * (2 * kTailDiv + 4) + 4) * n_sc;
@@ -1129,6 +1190,61 @@ static void fill_args(imager_plan* pl, TiledState* st, TiledArgs& a, const float
     a.gu_set = st->d_gu_set;
 }
 
+// imager_index_stats: sums over the sorted kept visibilities.  out: [0] sum S^2 of all kept, [1] sum S^2 of those that
+// are not merged duplicates, [2] merged duplicates.  sgeo == nullptr (no tiled plan yet): nothing is merged.
+__global__ void index_stats_kernel(const int32_t* __restrict__ counters, const int32_t* __restrict__ perm,
+                                   const imager_record* __restrict__ rec, const int32_t* __restrict__ set_support,
+                                   const uint2* __restrict__ sgeo, unsigned long long* __restrict__ out) {
+    const int n_kept = counters[0];
+    unsigned long long all = 0, own = 0, merged = 0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_kept; i += gridDim.x * blockDim.x) {
+        const unsigned long long S = (unsigned long long)set_support[rec[perm[i]].kset];
+        const bool m = sgeo && (sgeo[i].x & kMergedFlag);
+        all += S * S;
+        own += m ? 0ull : S * S;
+        merged += m ? 1ull : 0ull;
+    }
+    for (int d = 16; d > 0; d >>= 1) {
+        all += __shfl_xor_sync(0xffffffffu, all, d);
+        own += __shfl_xor_sync(0xffffffffu, own, d);
+        merged += __shfl_xor_sync(0xffffffffu, merged, d);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicAdd(out + 0, all);
+        atomicAdd(out + 1, own);
+        atomicAdd(out + 2, merged);
+    }
+}
+
+int tiled_index_stats(imager_plan* pl, int64_t out[8], cudaStream_t stream) {
+    TiledState* st = pl->tiled ? static_cast<TiledState*>(pl->tiled) : nullptr;
+    const bool planned = st && st->initialised && st->plan_epoch == pl->index_epoch;
+    unsigned long long* d_out = nullptr;
+    IMAGER_CUDA(cudaMalloc(&d_out, 3 * sizeof(unsigned long long)));
+    cudaError_t e = cudaMemsetAsync(d_out, 0, 3 * sizeof(unsigned long long), stream);
+    unsigned long long h[3] = {0, 0, 0};
+    int32_t c[2] = {0, 0};
+    if (e == cudaSuccess) {
+        index_stats_kernel<<<4 * kNumSMs, 256, 0, stream>>>(pl->d_counters, pl->d_perm[pl->sorted_buf], pl->d_rec,
+                                                            pl->d_set_support, planned ? st->d_sgeo : nullptr, d_out);
+        e = cudaMemcpyAsync(h, d_out, sizeof(h), cudaMemcpyDeviceToHost, stream);
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(c, pl->d_counters, sizeof(c), cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+    cudaFree(d_out);
+    if (e != cudaSuccess) return cuda_fail(e, "imager_index_stats");
+    const int64_t n_sc = (int64_t)pl->p.n_corr * pl->p.n_pol;
+    out[0] = c[0];
+    out[1] = c[1];
+    out[2] = (int64_t)h[2];
+    out[3] = n_sc * (int64_t)h[0];
+    out[4] = n_sc * (int64_t)h[1];
+    out[5] = planned ? st->h_totals[0] : 0;
+    out[6] = planned ? (int64_t) * reinterpret_cast<int32_t*>(&st->h_totals[1]) : 0;
+    out[7] = 0;
+    return 0;
+}
+
 // hit lists for the current index (imager_index: planning ahead of the first gridding / degridding call)
 int tiled_prepare(imager_plan* pl, int64_t nvis, cudaStream_t stream) {
     if (nvis == 0) return 0;
@@ -1155,9 +1271,9 @@ int launch_grid_tiled(imager_plan* pl, int64_t nvis, const float2* vis, const fl
     TiledArgs a;
     fill_args(pl, st, a, pl->d_tab_grid);
     if (pl->p.n_corr == 1)
-        grid_tiled_kernel<1><<<kNumSMs, kGridThreads, st->smem_bytes - kStageBytes + kGridStageBytes, stream>>>(a, st->d_sval, grid);
+        grid_tiled_kernel<1><<<kNumSMs, kGridThreads, st->smem_bytes + kGridStageBytes, stream>>>(a, st->d_sval, grid);
     else
-        grid_tiled_kernel<4><<<kNumSMs, kGridThreads, st->smem_bytes - kStageBytes + kGridStageBytes, stream>>>(a, st->d_sval, grid);
+        grid_tiled_kernel<4><<<kNumSMs, kGridThreads, st->smem_bytes + kGridStageBytes, stream>>>(a, st->d_sval, grid);
     pl->last_launches += 2;
     IMAGER_CUDA(cudaGetLastError());
     return 0;
@@ -1173,7 +1289,7 @@ int launch_degrid_tiled(imager_plan* pl, int64_t nvis, const float2* grid, float
     IMAGER_CUDA(cudaMemsetAsync(pl->d_counters + 8, 0, sizeof(int32_t), stream));
     TiledArgs a;
     fill_args(pl, st, a, pl->d_tab_degrid);
-    const int smem = st->smem_bytes + kRedBytes;
+    const int smem = st->smem_bytes + kStageBytes + kRedBytes;
     const unsigned gb = 4 * kNumSMs;
     if (nc == 1) {
         degrid_tiled_kernel<1><<<kNumSMs, kTiledThreads, smem, stream>>>(a, grid, st->d_sval);

@@ -6,6 +6,9 @@
 //       i = floor((q + O/2)/O), o = q - i*O, g = i + N/2;  p = min(P-1, rint(|w| * w_scale)), sp = sign(w) p
 //       kset = a*(2P-1) + sp + P-1;  drop if the S_p footprint leaves the grid
 //       key  = ((kset*nt + gy/32)*nt + gx/32)*O*O + (oy+O/2)*O + (ox+O/2), dropped -> 0xFFFFFFFF
+//       R17: non-finite u, v, w, |q| >= 2^30 or a_index outside [0, n_aplanes) -> dropped, record (0, 0, drop, 0)
+//     Internally the drop key is n_buckets * O * O (one more than the largest valid key), so that the radix sort needs
+//     only ceil(bits(n_buckets * O * O) / 8) passes; imager_debug_index exports it as 0xFFFFFFFF (the oracle's KEY_DROP).
 // A2: stable LSD radix sort (8-bit digits) of (key, input index), then dense bucket offsets by binary search.
 //     The sort is hand-written: per-warp chunk histograms -> exclusive scan -> stable per-warp scatter using
 //     __match_any_sync ranks.  Stability makes the permutation unique, hence comparable bit-exactly.
@@ -19,14 +22,30 @@ __device__ __forceinline__ long long floor_div(long long a, long long b) {
 }
 
 __global__ void index_kernel(int64_t nvis, const float* __restrict__ uvw, const int32_t* __restrict__ a_index,
-                             double uv_scale, double w_scale, int N, int O, int P, int nt,
+                             double uv_scale, double w_scale, int N, int O, int P, int nt, int n_aplanes, uint32_t key_drop,
                              const int32_t* __restrict__ plane_support, imager_record* __restrict__ rec,
                              uint32_t* __restrict__ key, int32_t* __restrict__ perm, int32_t* __restrict__ counters) {
     int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= nvis) return;
-    const float u = uvw[3 * k], v = uvw[3 * k + 1], w = uvw[3 * k + 2];
-    const long long qx = __double2ll_rn(__dmul_rn((double)u, uv_scale));
-    const long long qy = __double2ll_rn(__dmul_rn((double)v, uv_scale));
+    float u = uvw[3 * k], v = uvw[3 * k + 1], w = uvw[3 * k + 2];
+    int a = a_index ? a_index[k] : 0;
+    const double su = __dmul_rn((double)u, uv_scale), sv = __dmul_rn((double)v, uv_scale);
+    // R17: values that cannot be indexed are dropped before any cell or kernel-set index is formed from them
+    const bool invalid = !(isfinite(u) && isfinite(v) && isfinite(w)) || !(fabs(su) < 1073741824.0) ||
+                         !(fabs(sv) < 1073741824.0) || a < 0 || a >= n_aplanes;
+    if (invalid) {
+        imager_record r;
+        r.gx = r.gy = 0;
+        r.sub = 1u << 16;
+        r.kset = 0;
+        rec[k] = r;
+        atomicAdd(&counters[1], 1);
+        key[k] = key_drop;
+        perm[k] = (int32_t)k;
+        return;
+    }
+    const long long qx = __double2ll_rn(su);
+    const long long qy = __double2ll_rn(sv);
     const int half_o = O / 2;
     const long long ix = floor_div(qx + half_o, O), iy = floor_div(qy + half_o, O);
     const int ox = (int)(qx - ix * O), oy = (int)(qy - iy * O);
@@ -34,7 +53,6 @@ __global__ void index_kernel(int64_t nvis, const float* __restrict__ uvw, const 
     long long p = __double2ll_rn(__dmul_rn(fabs((double)w), w_scale));
     if (p > P - 1) p = P - 1;
     const int sp = (w < 0.f) ? -(int)p : (int)p;
-    const int a = a_index ? a_index[k] : 0;
     const int kset = a * (2 * P - 1) + sp + P - 1;
     const int S = plane_support[p], h_lo = S / 2, h_hi = S - 1 - h_lo;
     const bool drop = (gx - h_lo < 0) || (gx + h_hi >= N) || (gy - h_lo < 0) || (gy + h_hi >= N);
@@ -44,7 +62,7 @@ __global__ void index_kernel(int64_t nvis, const float* __restrict__ uvw, const 
     r.sub = (uint32_t)(ox + half_o) | ((uint32_t)(oy + half_o) << 8) | ((uint32_t)drop << 16);
     r.kset = kset;
     rec[k] = r;
-    uint32_t kk = kKeyDrop;
+    uint32_t kk = key_drop;
     if (!drop)
         kk = (uint32_t)((((long long)kset * nt + gy / kBucketTile) * nt + gx / kBucketTile) * (O * O) +
                         (oy + half_o) * O + (ox + half_o));
@@ -175,7 +193,7 @@ __global__ void bucket_offset_kernel(const uint32_t* __restrict__ skey, int64_t 
     int64_t lo = 0, hi = n;
     while (lo < hi) {
         const int64_t mid = (lo + hi) >> 1;
-        if ((uint64_t)skey[mid] < edge && skey[mid] != kKeyDrop) lo = mid + 1; else hi = mid;
+        if ((uint64_t)skey[mid] < edge) lo = mid + 1; else hi = mid;      // the drop key equals the last edge
     }
     bucket_offset[b] = (int32_t)lo;
     if (b == n_buckets) counters[0] = (int32_t)lo;      // n_kept
@@ -186,8 +204,8 @@ int run_index_and_sort(imager_plan* pl, int64_t nvis, const float* uvw, const in
     IMAGER_CUDA(cudaMemsetAsync(pl->d_counters, 0, 64 * sizeof(int32_t), st));
     if (nvis > 0) {
         index_kernel<<<(unsigned)((nvis + 255) / 256), 256, 0, st>>>(
-            nvis, uvw, a_index, pl->uv_scale, pl->w_scale, p.grid_size, p.oversample, p.n_wplanes, pl->nt,
-            pl->d_plane_support, pl->d_rec, pl->d_key[0], pl->d_perm[0], pl->d_counters);
+            nvis, uvw, a_index, pl->uv_scale, pl->w_scale, p.grid_size, p.oversample, p.n_wplanes, pl->nt, p.n_aplanes,
+            pl->key_drop, pl->d_plane_support, pl->d_rec, pl->d_key[0], pl->d_perm[0], pl->d_counters);
         pl->last_launches++;
     }
     int cur = 0;

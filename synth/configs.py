@@ -6,6 +6,11 @@ measurement sets (ASKAP / ALMA) are not available, so these stand i
 Draw order (numpy `default_rng(seed)`): antenna radii, antenna azimuths, leakage phases,
 visibilities.  uvw: textbook ENU -> (u, v, w) rotation for latitude phi, declination delta,
 hour angle H, scaled by nu/c per channel, cast to float32, order [time][baseline][channel].
+
+Chunks: `make_workload(name, time_range=(t0, t1))` builds only the (strided) time steps t0 <= t < t1 of an ASKAP-like
+workload (configs 2, 3, 5) with the cell size, w_max and parallactic-angle bins of the FULL track; the chunk's
+visibilities come from their own generator, `default_rng([seed, t0])`, so that config 5 (181 M visibilities x 4
+correlations, 11.6 GB of inputs) can be produced and fed chunk by chunk without ever being held whole.
 """
 from __future__ import annotations
 
@@ -83,7 +88,7 @@ def _cell_from_uv(uvw: np.ndarray, n: int) -> float:
 
 
 def _askap_like(name, seed, n_time, n_chan, hours, grid, n_corr, n_wplanes, smin, smax, mode,
-                n_aplanes, time_stride):
+                n_aplanes, time_stride, time_range=None):
     rng = np.random.default_rng(seed)
     lat, dec = -26.7, -30.0
     bx, by, bz = _array_xyz(36, 3000.0, lat, rng)
@@ -98,6 +103,9 @@ def _askap_like(name, seed, n_time, n_chan, hours, grid, n_corr, n_wplanes, smin
         wmax = max(wmax, float(np.abs(t[..., 2]).max()))
     cell = 1.0 / (grid * (umax / (0.4 * grid)))
     hs_used = hs[::time_stride]
+    t0, t1 = (0, len(hs_used)) if time_range is None else (int(time_range[0]), min(int(time_range[1]), len(hs_used)))
+    n_time_all = len(hs_used)
+    hs_used = hs_used[t0:t1]
     uvw = np.concatenate([uvw_tracks(bx, by, bz, dec, hs_used[a:a + 25], freqs).reshape(-1, 3)
                           for a in range(0, len(hs_used), 25)])
     nvis = uvw.shape[0]
@@ -108,9 +116,9 @@ def _askap_like(name, seed, n_time, n_chan, hours, grid, n_corr, n_wplanes, smin
         width = (hi - lo) / n_aplanes
         bins = np.minimum(n_aplanes - 1, np.floor((chi - lo) / width).astype(np.int64))
         pa_centres = lo + (np.arange(n_aplanes) + 0.5) * width
-        per_time = bins[::time_stride].astype(np.int32)
+        per_time = bins[::time_stride][t0:t1].astype(np.int32)
         a_index = np.repeat(per_time, bx.size * n_chan)
-    vis = _normal_vis(rng, nvis, n_corr)
+    vis = _normal_vis(rng if time_range is None else np.random.default_rng([seed, t0]), nvis, n_corr)
     params = dict(grid_size=grid, cell_size_rad=cell, n_corr=n_corr, n_pol=n_corr, n_wplanes=n_wplanes,
                   w_max=wmax, support_min=smin, support_max=smax, oversample=4, n_aplanes=n_aplanes,
                   kernel_mode=mode, dish_diameter_m=12.0, freq_hz=1.0e9,
@@ -118,7 +126,7 @@ def _askap_like(name, seed, n_time, n_chan, hours, grid, n_corr, n_wplanes, smin
                   pa_rad=[float(x) for x in pa_centres], pointing_lm=[[0.0, 0.0]] * n_aplanes,
                   pswf_support=7)
     return Workload(name, params, uvw, vis, np.ones((nvis, n_corr), np.float32), a_index,
-                    notes=dict(n_time=len(hs_used), n_chan=n_chan, n_baselines=int(bx.size), umax=umax))
+                    notes=dict(n_time=len(hs_used), n_time_all=n_time_all, n_chan=n_chan, n_baselines=int(bx.size), umax=umax))
 
 
 def _hex_pointings(n_point: int, spacing: float) -> np.ndarray:
@@ -171,19 +179,22 @@ def _config4(seed, time_stride):
 CONFIGS = ("config1", "config2", "config3", "config4", "config5")
 
 
-def make_workload(name: str, seed: int = 0, time_stride: int = 1) -> Workload:
+def make_workload(name: str, seed: int = 0, time_stride: int = 1, time_range=None) -> Workload:
     """Build one of the five workloads.  `time_stride` > 1 keeps every n-th time step (a smaller
-    workload with the same geometry, cell size and w_max) for tests and bounded CPU samples."""
+    workload with the same geometry, cell size and w_max) for tests and bounded CPU samples; `time_range` = (t0, t1)
+    keeps the (strided) time steps t0 <= t < t1 only (configs 2, 3, 5: chunked feeding, see the module docstring)."""
+    if time_range is not None and name not in ("config2", "config3", "config5"):
+        raise ValueError("time_range applies to the ASKAP-like workloads only")
     if name == "config1":
         return _config1(seed)
     if name == "config2":
-        return _askap_like("config2_wproj", seed, 300, 64, 8.0, 2048, 1, 32, 15, 63, MODE_WPROJ, 1, time_stride)
+        return _askap_like("config2_wproj", seed, 300, 64, 8.0, 2048, 1, 32, 15, 63, MODE_WPROJ, 1, time_stride, time_range)
     if name == "config3":
         return _askap_like("config3_aproj", seed, 300, 64, 8.0, 4096, 4, 8, 31, 31, MODE_AWPROJ_ADJOINT, 4,
-                           time_stride)
+                           time_stride, time_range)
     if name == "config4":
         return _config4(seed, time_stride)
     if name == "config5":
         return _askap_like("config5_major", seed, 1000, 288, 8.0, 8192, 4, 64, 15, 127, MODE_AWPROJ_ADJOINT, 4,
-                           time_stride)
+                           time_stride, time_range)
     raise ValueError(f"unknown workload {name!r}")

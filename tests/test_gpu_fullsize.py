@@ -1,9 +1,11 @@
 """GPU parity at BASELINE.json's full sizes (-m gpu), in the launch configuration bench.py times (default path,
-library called through the binding), on SAMPLED outputs the oracle computes one by one:
+library called through the binding):
   * index records, sorted keys, permutation, bucket offsets: bit-exact over ALL visibilities;
-  * 4000 grid cells (half of them at visibility positions, half uniformly in the uv coverage) and 4000 degridded
-    visibilities within 1e-5 of the oracle, normalised by sum |kernel . vis|.
-config5 (181 M visibilities, 3.2 GB of tables) is run with every 20th time step (marked slow: ~4 minutes)."""
+  * configs 1, 2, 4: EVERY grid cell and EVERY degridded visibility within 1e-5 of the oracle, normalised by
+    sum |kernel . vis| (block splitting, the two-ended queue and multi-group units only occur at these sizes);
+  * config 3 (1.9e11 complex MACs: 20 core-minutes of oracle): 4000 sampled grid cells (half of them at visibility
+    positions, half uniformly in the uv coverage) and 4000 sampled visibilities, which the oracle computes one by one.
+config 5 at its full size is tests/test_gpu_config5.py."""
 import numpy as np
 import pytest
 
@@ -14,7 +16,7 @@ pytestmark = pytest.mark.gpu
 TOL = 1e-5
 
 
-def _run(name, time_stride, n_samples=4000):
+def _run(name, time_stride, n_samples=4000, every_output=False):
     import torch
     assert torch.cuda.is_available()
     from paper_2206_15117_b200 import Plan
@@ -42,6 +44,24 @@ def _run(name, time_stride, n_samples=4000):
         grid = torch.zeros((npol, n, n), dtype=torch.complex64, device="cuda")
         plan.grid(uvw, vis, wts, grid, a, flags=1)
         torch.cuda.synchronize()
+        if every_output:
+            ref = og.grid(rec, wl.vis, wl.weights, flat, offs, params)
+            g = grid.cpu().numpy()
+            touched = ref["norm"] > 0
+            assert np.all(g[~touched] == 0)
+            err = np.max(np.abs(g[touched] - ref["grid"][touched]) / ref["norm"][touched])
+            assert err <= TOL, f"{name}: all-cell grid parity {err:.3e}"
+            del ref
+            out = torch.empty((nvis, nc), dtype=torch.complex64, device="cuda")
+            plan.degrid(uvw, grid, out, a, flags=1)
+            torch.cuda.synchronize()
+            refd = og.degrid(rec, g, flat, offs, params)
+            v = out.cpu().numpy()
+            ok = refd["norm"] > 0
+            errd = np.max(np.abs(v[ok] - refd["vis"][ok]) / refd["norm"][ok])
+            assert errd <= TOL, f"{name}: all-visibility degrid parity {errd:.3e}"
+            assert np.all(v[rec["drop"]] == 0)
+            return
         # sampled cells
         pick = rng.integers(0, nvis, n_samples // 2)
         near = np.stack([rec["gy"][pick] + rng.integers(-3, 4, pick.size), rec["gx"][pick] + rng.integers(-3, 4, pick.size)], 1)
@@ -71,16 +91,10 @@ def _run(name, time_stride, n_samples=4000):
         assert np.all(v[sub["drop"]] == 0)
 
 
-@pytest.mark.parametrize("name", ["config1", "config2", "config3", "config4"])
-def test_full_size_sampled_parity(oracle_lib, name):
-    _run(name, 1)
+@pytest.mark.parametrize("name", ["config1", "config2", "config4"])
+def test_full_size_every_output(oracle_lib, name):
+    _run(name, 1, every_output=True)
 
 
-@pytest.mark.slow
-def test_config5_strided_sampled_parity(oracle_lib):
-    """config5 with every 20th time step (9.07 M visibilities x 4 correlations, 8192^2 x 4 grids, supports up to 127,
-    3.2 GB of tables): about 4 minutes, most of it the oracle building its tables.  IMAGER_SKIP_SLOW=1 skips it."""
-    import os
-    if os.environ.get("IMAGER_SKIP_SLOW") == "1":
-        pytest.skip("IMAGER_SKIP_SLOW=1")
-    _run("config5", 20, n_samples=2000)
+def test_full_size_sampled_parity_config3(oracle_lib):
+    _run("config3", 1)

@@ -83,12 +83,17 @@ def test_transform_roundtrip_and_dirty_image():
         ref_grid = oi.image_to_grid(img_host.astype(np.complex128))
         assert np.abs(back.cpu().numpy()[0] - ref_grid).max() < 1e-4 * np.abs(ref_grid).max()
         # both directions divide by the taper (A4 corrects the dirty image, A5 pre-corrects the model image), so
-        # image -> grid -> image returns image / psi^2, not the identity
-        plan.grid_image_transform(back, +1, float(n * n))
-        expect = img_host / oi.taper_image(n) ** 2
-        # the pre-corrected image is huge at the field edge (psi(+-1) = 1.9e-4), and an fp32 FFT spreads its
-        # rounding error over every pixel: the bound is relative to the largest value that went through it
-        assert np.abs(back.cpu().numpy()[0] - expect)[inner].max() < 1e-5 * np.abs(expect).max()
+        # image -> grid -> image returns image / psi^2, not the identity.  The model is what a clean model is: zero
+        # outside the inner half (the pre-correction 1 / psi is 5e3 at the field edge and would swamp an fp32 FFT).
+        model = np.zeros((1, n, n), np.complex64)
+        model[0][inner] = img_host[inner]
+        rt = torch.from_numpy(model).cuda()
+        plan.grid_image_transform(rt, -1)
+        ref_model_grid = oi.image_to_grid(model[0].astype(np.complex128))
+        assert np.abs(rt.cpu().numpy()[0] - ref_model_grid).max() < 1e-5 * np.abs(ref_model_grid).max()
+        plan.grid_image_transform(rt, +1, float(n * n))
+        expect = model[0] / oi.taper_image(n) ** 2
+        assert np.abs(rt.cpu().numpy()[0] - expect)[inner].max() < 1e-4 * np.abs(expect[inner]).max()
 
 
 def test_end_to_end_with_library_tables_close_to_oracle():
