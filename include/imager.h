@@ -154,6 +154,41 @@ int imager_grid_image_transform(imager_plan* plan, float* data, int32_t directio
  * MOSAIC_PB mode), NOMEM, CUDA. */
 int imager_mosaic_correct(imager_plan* plan, float* image, void* cuda_stream);
 
+/* ---- the loop around the hot path: minor cycle and Cotton-Schwab major cycles ---- */
+
+/* Hogbom minor cycle (R18, R19) on device images, all float32 [n][n] row-major: `residual` is updated in
+ * place, `psf` has its peak (1) at pixel (n/2, n/2), the components found are ADDED to `model`.  window = {y0, x0, y1, x1}
+ * (half-open) limits the peak search.  Repeats up to n_iter times: p = first pixel (row-major) of the window with the
+ * largest |residual|; stop if |residual[p]| < max(threshold, cycle_factor * sidelobe * |first peak|), sidelobe = the largest
+ * |psf| outside the 3 x 3 pixels at its centre; a = gain * residual[p]; model[p] += a; residual[q] -= a * psf[q - p + c]
+ * wherever that psf sample exists.  Each step is one IEEE float32 operation (no fused multiply-add), so that peak positions
+ * and component values are reproducible bit for bit.  components_out dev float32 [n_iter][3] = (y, x, a) in the order
+ * found, or NULL; n_components_out dev int32 [1] or NULL.  Enqueues 2 n_iter + 3 kernels on cuda_stream; the stop test is
+ * taken on the device, nothing is read back and nothing synchronises.  Errors: INVALID_ARG, NOMEM, CUDA. */
+int imager_hogbom(float* residual, const float* psf, float* model, int32_t n, const int32_t window[4], float gain,
+                  float threshold, float cycle_factor, int32_t n_iter, float* components_out, int32_t* n_components_out,
+                  void* cuda_stream);
+
+typedef struct imager_clean_params {
+    int32_t n_major;          /* major (Cotton-Schwab) cycles, >= 1 ("number of clean cycles")                      */
+    int32_t n_iter;           /* minor-cycle iterations per major cycle                                                    */
+    float gain;               /* loop gain                                                                          */
+    float threshold;          /* stop level in image units                                                          */
+    float cycle_factor;       /* R19: a minor cycle ends at cycle_factor * PSF sidelobe * its first peak            */
+} imager_clean_params;
+
+/* Cotton-Schwab loop (R20) for single-polarisation plans: indexes (uvw, a_index) once, forms the PSF as the
+ * dirty image of unit visibilities, then n_major times: grids the residual visibilities (imager_grid, index reused),
+ * transforms (cuFFT + taper), runs the minor cycle inside the inner half of the field, transforms the accumulated model
+ * back and subtracts its prediction from the observed visibilities (imager_degrid with IMAGER_DEGRID_RESIDUAL).
+ * vis, weights dev [nvis]; model_image dev float32 [N][N] (overwritten: the clean components); residual_image dev float32
+ * [N][N] (the last cycle's image after its minor cycle); residual_vis dev complex64 [nvis] (V - V_model after the last
+ * cycle); psf_out dev float32 [N][N] or NULL; n_components_out dev int32 [n_major] or NULL.  Synchronises once (the
+ * indexing step); everything else is enqueued.  Errors: INVALID_ARG, UNSUPPORTED (n_pol != 1), TOO_MANY_VIS, NOMEM, CUDA. */
+int imager_clean(imager_plan* plan, int64_t nvis, const float* uvw, const float* vis, const float* weights,
+                 const int32_t* a_index, const imager_clean_params* params, float* model_image, float* residual_image,
+                 float* residual_vis, float* psf_out, int32_t* n_components_out, void* cuda_stream);
+
 /* ---- test / debug exports (synchronise; not part of the hot path) ---- */
 
 /* Runs indexing + bucketing for (uvw, a_index) and copies out: records host [nvis], perm host int32 [nvis]

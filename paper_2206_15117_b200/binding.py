@@ -22,7 +22,7 @@ DEGRID_RESIDUAL = 16
 
 EXPORTS = ("imager_plan_create", "imager_index", "imager_grid", "imager_degrid", "imager_plan_destroy",
            "imager_grid_image_transform", "imager_mosaic_correct", "imager_debug_index", "imager_debug_kernels", "imager_plan_info",
-           "imager_index_stats",
+           "imager_index_stats", "imager_hogbom", "imager_clean",
            "imager_last_launch_count", "imager_last_error")
 
 
@@ -37,6 +37,10 @@ class ImagerParams(Structure):
                 ("dish_diameter_m", c_double), ("freq_hz", c_double), ("leakage", c_double * 4), ("beam_eps", c_double),
                 ("pa_rad", POINTER(c_double)), ("pointing_lm", POINTER(c_double)), ("user_tables", POINTER(c_float)),
                 ("user_tables_degrid", POINTER(c_float)), ("max_nvis", c_int64)]
+
+
+class ImagerCleanParams(Structure):
+    _fields_ = [("n_major", c_int32), ("n_iter", c_int32), ("gain", c_float), ("threshold", c_float), ("cycle_factor", c_float)]
 
 
 _lib = None
@@ -64,6 +68,10 @@ def load_library() -> ctypes.CDLL:
     lib.imager_debug_kernels.argtypes = [c_void_p, c_int32, c_int32, c_void_p, POINTER(c_int32)]
     lib.imager_plan_info.argtypes = [c_void_p, POINTER(c_int64)]
     lib.imager_index_stats.argtypes = [c_void_p, POINTER(c_int64), c_void_p]
+    lib.imager_hogbom.argtypes = [c_void_p, c_void_p, c_void_p, c_int32, POINTER(c_int32), c_float, c_float, c_float, c_int32,
+                                  c_void_p, c_void_p, c_void_p]
+    lib.imager_clean.argtypes = [c_void_p, c_int64, c_void_p, c_void_p, c_void_p, c_void_p, POINTER(ImagerCleanParams), c_void_p,
+                                 c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
     lib.imager_last_launch_count.argtypes = [c_void_p]
     _lib = lib
     return lib
@@ -188,6 +196,18 @@ class Plan:
         _check(load_library().imager_mosaic_correct(self._h, _dev_ptr(image, torch.complex64, "image"), _stream_ptr(stream)),
                "imager_mosaic_correct")
 
+    def clean(self, uvw, vis, weights, model_image, residual_image, residual_vis, n_major: int, n_iter: int, gain: float,
+              threshold: float, cycle_factor: float, a_index=None, psf_out=None, n_components_out=None, stream=None):
+        """imager_clean: Cotton-Schwab major cycles around the hot path (single-polarisation plans)."""
+        import torch
+        cp = ImagerCleanParams(int(n_major), int(n_iter), float(gain), float(threshold), float(cycle_factor))
+        _check(load_library().imager_clean(
+            self._h, int(uvw.shape[0]), _dev_ptr(uvw, torch.float32, "uvw"), _dev_ptr(vis, torch.complex64, "vis"),
+            _dev_ptr(weights, torch.float32, "weights"), _dev_ptr(a_index, torch.int32, "a_index"), byref(cp),
+            _dev_ptr(model_image, torch.float32, "model_image"), _dev_ptr(residual_image, torch.float32, "residual_image"),
+            _dev_ptr(residual_vis, torch.complex64, "residual_vis"), _dev_ptr(psf_out, torch.float32, "psf_out"),
+            _dev_ptr(n_components_out, torch.int32, "n_components_out"), _stream_ptr(stream)), "imager_clean")
+
     def last_launch_count(self) -> int:
         return int(load_library().imager_last_launch_count(self._h))
 
@@ -227,3 +247,15 @@ class Plan:
         _check(load_library().imager_debug_kernels(self._h, kset, which, out.ctypes.data_as(c_void_p), byref(s)),
                "imager_debug_kernels")
         return out
+
+
+def hogbom(residual, psf, model, window, gain: float, threshold: float, cycle_factor: float, n_iter: int, components_out=None,
+           n_components_out=None, stream=None):
+    """imager_hogbom: the minor cycle on float32 CUDA images [n][n]; window = (y0, x0, y1, x1)."""
+    import torch
+    n = int(residual.shape[-1])
+    win = (c_int32 * 4)(*[int(v) for v in window])
+    _check(load_library().imager_hogbom(
+        _dev_ptr(residual, torch.float32, "residual"), _dev_ptr(psf, torch.float32, "psf"), _dev_ptr(model, torch.float32, "model"),
+        n, win, float(gain), float(threshold), float(cycle_factor), int(n_iter), _dev_ptr(components_out, torch.float32, "components_out"),
+        _dev_ptr(n_components_out, torch.int32, "n_components_out"), _stream_ptr(stream)), "imager_hogbom")

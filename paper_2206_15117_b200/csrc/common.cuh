@@ -97,6 +97,7 @@ int build_tables(imager_plan* pl, const imager_params* user, cudaStream_t st);
 
 // transform.cu
 int grid_image_transform(imager_plan* pl, float2* data, int direction, double norm, cudaStream_t st);
+int grid_image_transform_dev(imager_plan* pl, float2* data, int direction, const double* norm_dev, cudaStream_t st);
 void destroy_transform(imager_plan* pl);
 int mosaic_correct(imager_plan* pl, float2* image, cudaStream_t st);
 

@@ -9,10 +9,12 @@
 
 namespace imager {
 
+// norm_dev (device, may be NULL) overrides `norm`: the sum of weights of a gridding call that is still in flight
 __global__ void flip_scale_kernel(float2* __restrict__ data, int N, const double* __restrict__ taper, int divide,
-                                  double norm) {
+                                  double norm, const double* __restrict__ norm_dev) {
     const int x = blockIdx.x * blockDim.x + threadIdx.x, y = blockIdx.y;
     if (x >= N) return;
+    if (norm_dev) norm = (*norm_dev == 0.0) ? 1.0 : *norm_dev;
     double f = ((x + y) & 1) ? -1.0 : 1.0;
     if (divide) f /= (taper[x] * taper[y] * norm);
     float2 v = data[(int64_t)y * N + x];
@@ -21,7 +23,17 @@ __global__ void flip_scale_kernel(float2* __restrict__ data, int N, const double
     data[(int64_t)y * N + x] = v;
 }
 
+static int transform_impl(imager_plan* pl, float2* data, int direction, double norm, const double* norm_dev, cudaStream_t st);
+
 int grid_image_transform(imager_plan* pl, float2* data, int direction, double norm, cudaStream_t st) {
+    return transform_impl(pl, data, direction, norm, nullptr, st);
+}
+
+int grid_image_transform_dev(imager_plan* pl, float2* data, int direction, const double* norm_dev, cudaStream_t st) {
+    return transform_impl(pl, data, direction, 1.0, norm_dev, st);
+}
+
+static int transform_impl(imager_plan* pl, float2* data, int direction, double norm, const double* norm_dev, cudaStream_t st) {
     const int N = pl->p.grid_size;
     if (direction != 1 && direction != -1) {
         set_error("direction must be +1 or -1");
@@ -31,10 +43,12 @@ int grid_image_transform(imager_plan* pl, float2* data, int direction, double no
         Pswf psi(pl->p.pswf_support > 0 ? pl->p.pswf_support : 7);
         std::vector<double> t(N);
         for (int x = 0; x < N; ++x) t[x] = psi(2.0 * (x - N / 2) / N);
-        IMAGER_CUDA(cudaMalloc(&pl->d_taper, N * sizeof(double)));
+        if (!pl->d_taper) IMAGER_CUDA(cudaMalloc(&pl->d_taper, N * sizeof(double)));
         IMAGER_CUDA(cudaMemcpy(pl->d_taper, t.data(), N * sizeof(double), cudaMemcpyHostToDevice));
         cufftHandle h;
         if (cufftPlan2d(&h, N, N, CUFFT_C2C) != CUFFT_SUCCESS) {
+            cudaFree(pl->d_taper);                            // a retry starts clean
+            pl->d_taper = nullptr;
             set_error("cufftPlan2d(%d) failed", N);
             return IMAGER_ERR_CUDA;
         }
@@ -50,13 +64,13 @@ int grid_image_transform(imager_plan* pl, float2* data, int direction, double no
     const dim3 grid((N + 255) / 256, N);
     for (int s = 0; s < pl->p.n_pol; ++s) {
         float2* plane = data + (int64_t)s * N * N;
-        flip_scale_kernel<<<grid, 256, 0, st>>>(plane, N, pl->d_taper, direction == -1, 1.0);
+        flip_scale_kernel<<<grid, 256, 0, st>>>(plane, N, pl->d_taper, direction == -1, 1.0, nullptr);
         if (cufftExecC2C(h, (cufftComplex*)plane, (cufftComplex*)plane, direction == 1 ? CUFFT_FORWARD : CUFFT_INVERSE) !=
             CUFFT_SUCCESS) {
             set_error("cufftExecC2C failed");
             return IMAGER_ERR_CUDA;
         }
-        flip_scale_kernel<<<grid, 256, 0, st>>>(plane, N, pl->d_taper, direction == 1, norm);
+        flip_scale_kernel<<<grid, 256, 0, st>>>(plane, N, pl->d_taper, direction == 1, norm, direction == 1 ? norm_dev : nullptr);
     }
     IMAGER_CUDA(cudaGetLastError());
     return 0;
