@@ -189,6 +189,39 @@ int imager_clean(imager_plan* plan, int64_t nvis, const float* uvw, const float*
                  const int32_t* a_index, const imager_clean_params* params, float* model_image, float* residual_image,
                  float* residual_vis, float* psf_out, int32_t* n_components_out, void* cuda_stream);
 
+/* ---- image-domain mosaic (R21-R23) ---- */
+
+/* Image-plane reprojection (R22): dst(l, m) (+)= B * bilinear(src at (l - shift_l, m - shift_m)), zero outside the source.
+ * src dev complex64 [n_src][n_src] with cell cell_src, dst dev complex64 [n_dst][n_dst] with cell cell_dst (radians), pixel
+ * (n/2, n/2) the origin of either frame, l along the last axis.  beam: 0 none, 1 = Airy power beam E^2 (dish_diameter_m,
+ * freq_hz) centred on the SOURCE frame (forward: component -> mosaic), 2 = centred on the TARGET frame (backward: model ->
+ * component).  inner_half != 0: only source pixels n/4 <= x, y < 3n/4 count.  accumulate != 0 adds to dst.  Enqueues one
+ * kernel.  Errors: INVALID_ARG, CUDA. */
+int imager_reproject(const float* src, int32_t n_src, double cell_src, float* dst, int32_t n_dst, double cell_dst,
+                     double shift_l, double shift_m, int32_t beam, double dish_diameter_m, double freq_hz, int32_t inner_half,
+                     int32_t accumulate, void* cuda_stream);
+
+/* Image-domain mosaic, forward (R23): every component i = 0 .. n_point-1 (visibilities referred to ITS OWN phase
+ * centre) is gridded on the plan's grid (imager_grid: index + bucket + grid), transformed (cuFFT + taper), weighted by the
+ * Airy power beam of the plan (dish_diameter_m, freq_hz) and reprojected to the mosaic frame at offset pointing_lm[i];
+ * mosaic_image = sum_i w_i B_i reproject_i[I_i], w_i = component i's sum of weights / the total.  `plan`: single
+ * polarisation, one A-plane, kernel mode PSWF or WPROJ.  nvis host [n_point]; uvw, vis, weights host arrays of n_point DEVICE
+ * pointers ([nvis_i][3] float32, [nvis_i] complex64, [nvis_i] float32); pointing_lm host [n_point][2] radians;
+ * mosaic_image dev complex64 [n_mosaic][n_mosaic] (OVERWRITTEN), cell_mosaic radians; sum_weights dev double [1] or NULL
+ * (the total).  Synchronises once per component (its indexing step).  Errors: INVALID_ARG, UNSUPPORTED, TOO_MANY_VIS
+ * (a component larger than max_nvis), NOMEM, CUDA. */
+int imager_mosaic_grid(imager_plan* plan, int32_t n_point, const int64_t* nvis, const float* const* uvw,
+                       const float* const* vis, const float* const* weights, const double* pointing_lm, float* mosaic_image,
+                       int32_t n_mosaic, double cell_mosaic, double* sum_weights, void* cuda_stream);
+
+/* Image-domain mosaic, backward ("the model image is reprojected to the phase position of each mosaic component, and
+ * multiple FFT and degridding steps are performed"): per component, model_image is reprojected to the component frame,
+ * multiplied by the beam, transformed to the grid (taper + cuFFT) and degridded at the component's uvw into vis_out[i]
+ * (dev complex64 [nvis_i]; flags: 0 or IMAGER_DEGRID_RESIDUAL).  Arguments as imager_mosaic_grid. */
+int imager_mosaic_degrid(imager_plan* plan, int32_t n_point, const int64_t* nvis, const float* const* uvw,
+                         const double* pointing_lm, const float* model_image, int32_t n_mosaic, double cell_mosaic,
+                         float* const* vis_out, uint32_t flags, void* cuda_stream);
+
 /* ---- test / debug exports (synchronise; not part of the hot path) ---- */
 
 /* Runs indexing + bucketing for (uvw, a_index) and copies out: records host [nvis], perm host int32 [nvis]

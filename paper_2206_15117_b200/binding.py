@@ -22,7 +22,8 @@ DEGRID_RESIDUAL = 16
 
 EXPORTS = ("imager_plan_create", "imager_index", "imager_grid", "imager_degrid", "imager_plan_destroy",
            "imager_grid_image_transform", "imager_mosaic_correct", "imager_debug_index", "imager_debug_kernels", "imager_plan_info",
-           "imager_index_stats", "imager_hogbom", "imager_clean",
+           "imager_index_stats", "imager_hogbom", "imager_clean", "imager_reproject", "imager_mosaic_grid",
+           "imager_mosaic_degrid",
            "imager_last_launch_count", "imager_last_error")
 
 
@@ -68,6 +69,12 @@ def load_library() -> ctypes.CDLL:
     lib.imager_debug_kernels.argtypes = [c_void_p, c_int32, c_int32, c_void_p, POINTER(c_int32)]
     lib.imager_plan_info.argtypes = [c_void_p, POINTER(c_int64)]
     lib.imager_index_stats.argtypes = [c_void_p, POINTER(c_int64), c_void_p]
+    lib.imager_reproject.argtypes = [c_void_p, c_int32, c_double, c_void_p, c_int32, c_double, c_double, c_double, c_int32,
+                                     c_double, c_double, c_int32, c_int32, c_void_p]
+    lib.imager_mosaic_grid.argtypes = [c_void_p, c_int32, POINTER(c_int64), POINTER(c_void_p), POINTER(c_void_p), POINTER(c_void_p),
+                                       POINTER(c_double), c_void_p, c_int32, c_double, c_void_p, c_void_p]
+    lib.imager_mosaic_degrid.argtypes = [c_void_p, c_int32, POINTER(c_int64), POINTER(c_void_p), POINTER(c_double), c_void_p,
+                                         c_int32, c_double, POINTER(c_void_p), c_uint32, c_void_p]
     lib.imager_hogbom.argtypes = [c_void_p, c_void_p, c_void_p, c_int32, POINTER(c_int32), c_float, c_float, c_float, c_int32,
                                   c_void_p, c_void_p, c_void_p]
     lib.imager_clean.argtypes = [c_void_p, c_int64, c_void_p, c_void_p, c_void_p, c_void_p, POINTER(ImagerCleanParams), c_void_p,
@@ -208,6 +215,34 @@ class Plan:
             _dev_ptr(residual_vis, torch.complex64, "residual_vis"), _dev_ptr(psf_out, torch.float32, "psf_out"),
             _dev_ptr(n_components_out, torch.int32, "n_components_out"), _stream_ptr(stream)), "imager_clean")
 
+    @staticmethod
+    def _ptr_array(tensors, dtype, what):
+        return (c_void_p * len(tensors))(*[_dev_ptr(t, dtype, what).value for t in tensors])
+
+    def mosaic_grid(self, uvw_list, vis_list, weights_list, pointing_lm, mosaic_image, cell_mosaic: float, sum_weights=None,
+                    stream=None):
+        """imager_mosaic_grid: image-domain mosaic of components given at their own phase centres (lists of CUDA tensors)."""
+        import torch
+        k = len(uvw_list)
+        nv = (c_int64 * k)(*[int(u.shape[0]) for u in uvw_list])
+        lm = np.ascontiguousarray(pointing_lm, dtype=np.float64).reshape(-1)
+        _check(load_library().imager_mosaic_grid(
+            self._h, k, nv, self._ptr_array(uvw_list, torch.float32, "uvw"), self._ptr_array(vis_list, torch.complex64, "vis"),
+            self._ptr_array(weights_list, torch.float32, "weights"), lm.ctypes.data_as(POINTER(c_double)),
+            _dev_ptr(mosaic_image, torch.complex64, "mosaic_image"), int(mosaic_image.shape[-1]), float(cell_mosaic),
+            _dev_ptr(sum_weights, torch.float64, "sum_weights"), _stream_ptr(stream)), "imager_mosaic_grid")
+
+    def mosaic_degrid(self, uvw_list, pointing_lm, model_image, cell_mosaic: float, vis_out_list, flags: int = 0, stream=None):
+        """imager_mosaic_degrid: predicts every component's visibilities from a model image on the mosaic frame."""
+        import torch
+        k = len(uvw_list)
+        nv = (c_int64 * k)(*[int(u.shape[0]) for u in uvw_list])
+        lm = np.ascontiguousarray(pointing_lm, dtype=np.float64).reshape(-1)
+        _check(load_library().imager_mosaic_degrid(
+            self._h, k, nv, self._ptr_array(uvw_list, torch.float32, "uvw"), lm.ctypes.data_as(POINTER(c_double)),
+            _dev_ptr(model_image, torch.complex64, "model_image"), int(model_image.shape[-1]), float(cell_mosaic),
+            self._ptr_array(vis_out_list, torch.complex64, "vis_out"), flags, _stream_ptr(stream)), "imager_mosaic_degrid")
+
     def last_launch_count(self) -> int:
         return int(load_library().imager_last_launch_count(self._h))
 
@@ -259,3 +294,13 @@ def hogbom(residual, psf, model, window, gain: float, threshold: float, cycle_fa
         _dev_ptr(residual, torch.float32, "residual"), _dev_ptr(psf, torch.float32, "psf"), _dev_ptr(model, torch.float32, "model"),
         n, win, float(gain), float(threshold), float(cycle_factor), int(n_iter), _dev_ptr(components_out, torch.float32, "components_out"),
         _dev_ptr(n_components_out, torch.int32, "n_components_out"), _stream_ptr(stream)), "imager_hogbom")
+
+
+def reproject(src, cell_src: float, dst, cell_dst: float, shift_lm, beam: int = 0, dish_diameter_m: float = 0.0,
+              freq_hz: float = 0.0, inner_half: bool = False, accumulate: bool = False, stream=None):
+    """imager_reproject: bilinear image-plane reprojection between complex64 CUDA images (R22)."""
+    import torch
+    _check(load_library().imager_reproject(
+        _dev_ptr(src, torch.complex64, "src"), int(src.shape[-1]), float(cell_src), _dev_ptr(dst, torch.complex64, "dst"),
+        int(dst.shape[-1]), float(cell_dst), float(shift_lm[0]), float(shift_lm[1]), int(beam), float(dish_diameter_m),
+        float(freq_hz), int(bool(inner_half)), int(bool(accumulate)), _stream_ptr(stream)), "imager_reproject")

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libimager.so")
-SOURCES = ["api.cu", "index_sort.cu", "gridder_ref.cu", "gridder_tiled.cu", "tables.cu", "transform.cu", "clean.cu"]
+SOURCES = ["api.cu", "index_sort.cu", "gridder_ref.cu", "gridder_tiled.cu", "tables.cu", "transform.cu", "clean.cu", "mosaic.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC",
               "-Xptxas", "-v"]
 
