@@ -11,7 +11,7 @@ namespace imager {
 
 constexpr int kBucketTile = 32;          // bucketing tile (cells); DESIGN.md "Bucketing key"
 constexpr uint32_t kKeyDrop = 0xFFFFFFFFu;   // exported key of a dropped visibility (the oracle's KEY_DROP)
-constexpr int kSortChunk = 2048;         // items per warp in the radix sort
+constexpr int kSortChunk = 4096;         // items per CTA tile in the radix sort
 constexpr int kNumSMs = 148;             // B200
 
 void set_error(const char* fmt, ...);
@@ -46,7 +46,7 @@ struct imager_plan {
     int32_t* d_perm[2] = {nullptr, nullptr};
     int sorted_buf = 0;                  // which of d_key/d_perm holds the sorted result
     int32_t* d_bucket_offset = nullptr;  // [n_buckets + 1]
-    int32_t* d_hist = nullptr;           // radix histograms [256 * n_warp_chunks]
+    int32_t* d_hist = nullptr;           // radix histograms [256 * n_tiles]
     int32_t* d_scan_tmp = nullptr;       // block sums of the scan, all levels
     int64_t scan_tmp_len = 0;
     int32_t* d_counters = nullptr;       // [0] n_kept, [1] n_dropped, [2..] work-queue heads

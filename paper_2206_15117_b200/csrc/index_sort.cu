@@ -10,8 +10,9 @@
 //     Internally the drop key is n_buckets * O * O (one more than the largest valid key), so that the radix sort needs
 //     only ceil(bits(n_buckets * O * O) / 8) passes; imager_debug_index exports it as 0xFFFFFFFF (the oracle's KEY_DROP).
 // A2: stable LSD radix sort (8-bit digits) of (key, input index), then dense bucket offsets by binary search.
-//     The sort is hand-written: per-warp chunk histograms -> exclusive scan -> stable per-warp scatter using
-//     __match_any_sync ranks.  Stability makes the permutation unique, hence comparable bit-exactly.
+//     The sort is hand-written: per-tile (4096 items, one CTA) histograms -> exclusive scan -> stable scatter: ranks from
+//     __match_any_sync within rows of 32 items, the tile sorted by digit in shared memory and written out in runs
+//     (coalesced).  Stability makes the permutation unique, hence comparable bit-exactly.
 #include "common.cuh"
 
 namespace imager {
@@ -24,7 +25,7 @@ __device__ __forceinline__ long long floor_div(long long a, long long b) {
 __global__ void index_kernel(int64_t nvis, const float* __restrict__ uvw, const int32_t* __restrict__ a_index,
                              double uv_scale, double w_scale, int N, int O, int P, int nt, int n_aplanes, uint32_t key_drop,
                              const int32_t* __restrict__ plane_support, imager_record* __restrict__ rec,
-                             uint32_t* __restrict__ key, int32_t* __restrict__ perm, int32_t* __restrict__ counters) {
+                             uint32_t* __restrict__ key, int32_t* __restrict__ counters) {   // the permutation starts as the identity: first sort pass
     int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= nvis) return;
     float u = uvw[3 * k], v = uvw[3 * k + 1], w = uvw[3 * k + 2];
@@ -41,7 +42,6 @@ __global__ void index_kernel(int64_t nvis, const float* __restrict__ uvw, const 
         rec[k] = r;
         atomicAdd(&counters[1], 1);
         key[k] = key_drop;
-        perm[k] = (int32_t)k;
         return;
     }
     const long long qx = __double2ll_rn(su);
@@ -69,56 +69,123 @@ __global__ void index_kernel(int64_t nvis, const float* __restrict__ uvw, const 
     else
         atomicAdd(&counters[1], 1);
     key[k] = kk;
-    perm[k] = (int32_t)k;
 }
 
-// ---- radix sort: one warp owns kSortChunk consecutive items ----
-__global__ void radix_hist_kernel(int64_t n, const uint32_t* __restrict__ key, int shift, int32_t* __restrict__ hist,
-                                  int n_chunks) {
-    __shared__ int32_t cnt[4][256];
+// ---- radix sort: one CTA owns a tile of kSortChunk consecutive items (8 warps x kSortRows rows of 32) ----
+constexpr int kSortThreads = 256, kSortWarps = kSortThreads / 32, kSortRows = kSortChunk / kSortThreads;
+
+__global__ void __launch_bounds__(kSortThreads) radix_hist_kernel(int64_t n, const uint32_t* __restrict__ key, int shift,
+                                                                  int32_t* __restrict__ hist, int n_tiles) {
+    __shared__ int32_t cnt[kSortWarps][256];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int chunk = blockIdx.x * 4 + warp;
+    const int tile = blockIdx.x;
     for (int i = lane; i < 256; i += 32) cnt[warp][i] = 0;
     __syncwarp();
-    if (chunk < n_chunks) {
-        const int64_t base = (int64_t)chunk * kSortChunk;
-        for (int i = lane; i < kSortChunk; i += 32) {
-            const int64_t idx = base + i;
-            if (idx < n) atomicAdd(&cnt[warp][(key[idx] >> shift) & 255u], 1);
-        }
-        __syncwarp();
-        for (int d = lane; d < 256; d += 32) hist[(int64_t)d * n_chunks + chunk] = cnt[warp][d];
+    const int64_t base = (int64_t)tile * kSortChunk + warp * (kSortRows * 32);
+#pragma unroll 4
+    for (int r = 0; r < kSortRows; ++r) {
+        const int64_t idx = base + r * 32 + lane;
+        if (idx < n) atomicAdd(&cnt[warp][(key[idx] >> shift) & 255u], 1);
     }
+    __syncthreads();
+    int t = 0;
+#pragma unroll
+    for (int w = 0; w < kSortWarps; ++w) t += cnt[w][threadIdx.x];
+    hist[(int64_t)threadIdx.x * n_tiles + tile] = t;
 }
 
-__global__ void radix_scatter_kernel(int64_t n, const uint32_t* __restrict__ key_in, const int32_t* __restrict__ val_in,
-                                     uint32_t* __restrict__ key_out, int32_t* __restrict__ val_out, int shift,
-                                     const int32_t* __restrict__ hist_scanned, int n_chunks) {
-    __shared__ int32_t pos[4][256];
+// Stable scatter of one tile.  Ranks: per row of 32 consecutive items the lanes with the same digit find each other with
+// __match_any_sync (rank = lower peers), per-warp digit counters order the rows, a prefix over the warps orders the
+// warps: the tile is first sorted by digit in shared memory, then written out in runs of equal digit (coalesced), each
+// run to the place the scanned histograms give it.  val_in == nullptr: the values are the input indices (first pass).
+__global__ void __launch_bounds__(kSortThreads) radix_scatter_kernel(int64_t n, const uint32_t* __restrict__ key_in,
+                                                                     const int32_t* __restrict__ val_in,
+                                                                     uint32_t* __restrict__ key_out, int32_t* __restrict__ val_out,
+                                                                     int shift, const int32_t* __restrict__ hist_scanned, int n_tiles) {
+    __shared__ int32_t wcount[kSortWarps][256];
+    __shared__ int32_t dstart[256], gdelta[256], wsum[kSortWarps];
+    __shared__ uint32_t s_key[kSortChunk];
+    __shared__ int32_t s_val[kSortChunk];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int chunk = blockIdx.x * 4 + warp;
-    if (chunk >= n_chunks) return;
-    for (int d = lane; d < 256; d += 32) pos[warp][d] = hist_scanned[(int64_t)d * n_chunks + chunk];
-    __syncwarp();
-    const int64_t base = (int64_t)chunk * kSortChunk;
+    const int tile = blockIdx.x;
     const unsigned lt_mask = (1u << lane) - 1u;
-    for (int i = 0; i < kSortChunk; i += 32) {
-        const int64_t idx = base + i + lane;
+    for (int i = lane; i < 256; i += 32) wcount[warp][i] = 0;
+    __syncwarp();
+    const int64_t base = (int64_t)tile * kSortChunk + warp * (kSortRows * 32);
+    uint32_t k[kSortRows];
+    int32_t v[kSortRows];
+    int32_t lrank[kSortRows];                   // rank of the item among those of its warp with the same digit
+#pragma unroll
+    for (int r = 0; r < kSortRows; ++r) {
+        const int64_t idx = base + r * 32 + lane;
+        k[r] = 0u;
+        v[r] = 0;
+        if (idx < n) {
+            k[r] = key_in[idx];
+            v[r] = val_in ? val_in[idx] : (int32_t)idx;
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < kSortRows; ++r) {
+        const int64_t idx = base + r * 32 + lane;
         const bool live = idx < n;
         const unsigned active = __ballot_sync(0xffffffffu, live);
+        lrank[r] = 0;
         if (live) {
-            const uint32_t kk = key_in[idx];
-            const int32_t vv = val_in[idx];
-            const unsigned d = (kk >> shift) & 255u;
+            const unsigned d = (k[r] >> shift) & 255u;
             const unsigned peers = __match_any_sync(active, d);
             const int rank = __popc(peers & lt_mask);
-            const int dst = pos[warp][d] + rank;
+            lrank[r] = wcount[warp][d] + rank;
             __syncwarp(active);
-            if (rank == 0) pos[warp][d] += __popc(peers);
-            key_out[dst] = kk;
-            val_out[dst] = vv;
+            if (rank == 0) wcount[warp][d] += __popc(peers);
         }
         __syncwarp();
+    }
+    __syncthreads();
+    {   // thread d: exclusive prefix of digit d over the warps, then of the digit totals over the digits
+        const int d = threadIdx.x;
+        int t = 0;
+#pragma unroll
+        for (int w = 0; w < kSortWarps; ++w) {
+            const int c = wcount[w][d];
+            wcount[w][d] = t;
+            t += c;
+        }
+        int inc = t;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int y = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += y;
+        }
+        if (lane == 31) wsum[warp] = inc;
+        __syncthreads();
+        int woff = 0;
+#pragma unroll
+        for (int w = 0; w < kSortWarps; ++w)
+            if (w < warp) woff += wsum[w];
+        const int start = woff + inc - t;
+        dstart[d] = start;
+        gdelta[d] = hist_scanned[(int64_t)d * n_tiles + tile] - start;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < kSortRows; ++r) {
+        const int64_t idx = base + r * 32 + lane;
+        if (idx < n) {
+            const unsigned d = (k[r] >> shift) & 255u;
+            const int pos = dstart[d] + wcount[warp][d] + lrank[r];
+            s_key[pos] = k[r];
+            s_val[pos] = v[r];
+        }
+    }
+    __syncthreads();
+    const int64_t left = n - (int64_t)tile * kSortChunk;
+    const int count = left < kSortChunk ? (int)left : kSortChunk;
+    for (int i = threadIdx.x; i < count; i += kSortThreads) {
+        const uint32_t kk = s_key[i];
+        const int dst = gdelta[(kk >> shift) & 255u] + i;
+        key_out[dst] = kk;
+        val_out[dst] = s_val[i];
     }
 }
 
@@ -205,20 +272,20 @@ int run_index_and_sort(imager_plan* pl, int64_t nvis, const float* uvw, const in
     if (nvis > 0) {
         index_kernel<<<(unsigned)((nvis + 255) / 256), 256, 0, st>>>(
             nvis, uvw, a_index, pl->uv_scale, pl->w_scale, p.grid_size, p.oversample, p.n_wplanes, pl->nt, p.n_aplanes,
-            pl->key_drop, pl->d_plane_support, pl->d_rec, pl->d_key[0], pl->d_perm[0], pl->d_counters);
+            pl->key_drop, pl->d_plane_support, pl->d_rec, pl->d_key[0], pl->d_counters);
         pl->last_launches++;
     }
     int cur = 0;
     const int n_chunks = (int)((nvis + kSortChunk - 1) / kSortChunk);
     for (int pass = 0; pass < pl->sort_passes && nvis > 0; ++pass) {
         const int shift = 8 * pass;
-        const unsigned blocks = (unsigned)((n_chunks + 3) / 4);
-        radix_hist_kernel<<<blocks, 128, 0, st>>>(nvis, pl->d_key[cur], shift, pl->d_hist, n_chunks);
+        const unsigned blocks = (unsigned)n_chunks;
+        radix_hist_kernel<<<blocks, kSortThreads, 0, st>>>(nvis, pl->d_key[cur], shift, pl->d_hist, n_chunks);
         pl->last_launches++;
         int rc = exclusive_scan(pl, pl->d_hist, (int64_t)256 * n_chunks, pl->d_scan_tmp, st);
         if (rc) return rc;
-        radix_scatter_kernel<<<blocks, 128, 0, st>>>(nvis, pl->d_key[cur], pl->d_perm[cur], pl->d_key[cur ^ 1],
-                                                     pl->d_perm[cur ^ 1], shift, pl->d_hist, n_chunks);
+        radix_scatter_kernel<<<blocks, kSortThreads, 0, st>>>(nvis, pl->d_key[cur], pass == 0 ? nullptr : pl->d_perm[cur],
+                                                              pl->d_key[cur ^ 1], pl->d_perm[cur ^ 1], shift, pl->d_hist, n_chunks);
         pl->last_launches++;
         cur ^= 1;
     }
