@@ -108,10 +108,10 @@ __global__ void sorted_geo_kernel(const int32_t* __restrict__ counters, const in
 constexpr int kDedupeChunk = 4096, kDedupeSlots = 8192;          // shared hash table: load factor <= 0.5
 constexpr int kDedupeSmem = kDedupeSlots * 12;
 constexpr uint32_t kMergedFlag = 0x8000u;                       // bit 15 of sgeo.x (gx < 2^15): merged into another one
-constexpr int kDedupeThreads = 256, kDedupePer = kDedupeChunk / kDedupeThreads;
+constexpr int kDedupeThreads = 1024, kDedupePer = kDedupeChunk / kDedupeThreads;   // 2 CTAs per SM: 64 warps hide the gather
 // Fused with the sorted-geometry pass: one CTA builds sgeo for kDedupeChunk consecutive sorted visibilities, finds their
 // representatives through a shared hash table (min sorted index per geometry) and flags the merged ones.
-__global__ void __launch_bounds__(kDedupeThreads) sorted_geo_dedupe_kernel(const int32_t* __restrict__ counters,
+__global__ void __launch_bounds__(kDedupeThreads, 2) sorted_geo_dedupe_kernel(const int32_t* __restrict__ counters,
                                                                            const int32_t* __restrict__ perm,
                                                                            const imager_record* __restrict__ rec, int O,
                                                                            uint2* __restrict__ sgeo, int32_t* __restrict__ rep) {
@@ -245,15 +245,16 @@ __device__ __forceinline__ uint32_t ctrl_variant(uint32_t ctrl) {
 }
 
 
-// Hit counts per (gu, strip), visibility-centric: every kept visibility adds 1 to each strip its footprint meets
-// (about 4 atomics per visibility; sorted order makes neighbouring threads meet the same few counters in L2).
-#ifndef IMAGER_AGGREGATE
-#define IMAGER_AGGREGATE 1
-#endif
-// the strips a kept visibility meets: cell index of its t-th hit, t = 0 .. n - 1 (row-major over the strips)
+// Hit counts per (gu, strip), visibility-centric and warp-aggregated.  The lanes of a warp hold 32 consecutive sorted
+// visibilities: mostly one kernel set and one or two neighbouring 32 x 32 tiles, so their footprints meet the same few
+// strips.  Per group of lanes with the same geometry unit the warp walks the bounding box of the group's strips (the
+// "window", at most kWindowMax strips) and counts the lanes that meet each strip with one ballot: no __match_any_sync
+// (the MIO queue was the limit of the match-based version: short_scoreboard 19.6, mio_throttle 15.8 stalls per issue),
+// one atomic per (warp, strip).  Lane t keeps the count of window strip t (and t + 32).
+constexpr int kWindowMax = 64;
+// the strips a kept visibility meets: sx0 .. sx0 + nsx - 1, sy0 .. sy0 + nsy - 1 of geometry unit gu
 struct VisHits {
-    int64_t cell0;      // (gu, strip (sy0, sx0))
-    int nsx, n, x0, y0, sx0, sy0, S, subl, kset;
+    int gu, nsx, nsy, n, x0, y0, sx0, sy0, S, subl, kset;
 };
 __device__ __forceinline__ VisHits vis_hits(const PlanArgs& a, const uint2 geo) {
     VisHits v;
@@ -269,9 +270,28 @@ __device__ __forceinline__ VisHits vis_hits(const PlanArgs& a, const uint2 geo) 
     v.sx0 = v.x0 / kStripW;
     v.sy0 = v.y0 / kStripH;
     v.nsx = (v.x0 + v.S - 1) / kStripW - v.sx0 + 1;
-    v.n = v.nsx * ((v.y0 + v.S - 1) / kStripH - v.sy0 + 1);
-    v.cell0 = (int64_t)(sp.gu_base + group) * a.g.n_strips + (int64_t)v.sy0 * a.g.strips_per_row + v.sx0;
+    v.nsy = (v.y0 + v.S - 1) / kStripH - v.sy0 + 1;
+    v.n = v.nsx * v.nsy;
+    v.gu = sp.gu_base + group;
     return v;
+}
+
+// One group of a warp's lanes (same geometry unit) and the window of strips they meet
+struct HitWindow {
+    unsigned group;            // lanes of the group
+    int gu, x_lo, y_lo, w, h;  // window = strips x_lo .. x_lo + w - 1, y_lo .. y_lo + h - 1
+};
+__device__ __forceinline__ HitWindow next_window(const VisHits& v, bool valid, unsigned pending) {
+    HitWindow win;
+    const int leader = __ffs(pending) - 1;
+    win.gu = __shfl_sync(0xffffffffu, v.gu, leader);
+    const bool mine = valid && v.gu == win.gu;
+    win.group = __ballot_sync(0xffffffffu, mine);
+    win.x_lo = __reduce_min_sync(0xffffffffu, mine ? v.sx0 : 0x7fffffff);
+    win.y_lo = __reduce_min_sync(0xffffffffu, mine ? v.sy0 : 0x7fffffff);
+    win.w = __reduce_max_sync(0xffffffffu, mine ? v.sx0 + v.nsx : 0) - win.x_lo;
+    win.h = __reduce_max_sync(0xffffffffu, mine ? v.sy0 + v.nsy : 0) - win.y_lo;
+    return win;
 }
 
 __global__ void count_hits_kernel(const PlanArgs a, const int32_t* __restrict__ counters, int32_t* __restrict__ hits,
@@ -279,35 +299,51 @@ __global__ void count_hits_kernel(const PlanArgs a, const int32_t* __restrict__ 
     const Geometry& g = a.g;
     const int n_kept = counters[0];
     const int lane = threadIdx.x & 31;
-    int mine = 0;                              // hits of this thread's visibilities (the 64-bit total guards the int32 scan)
-    // warp-uniform trip count: the lanes of a warp hold consecutive sorted visibilities, which mostly meet the same strips
+    int mine_total = 0;                        // hits of this thread's visibilities (the 64-bit total guards the int32 scan)
     for (int i0 = (blockIdx.x * blockDim.x + threadIdx.x) - lane; i0 < n_kept; i0 += gridDim.x * blockDim.x) {
         const int i = i0 + lane;
         VisHits v;
         v.n = 0;
+        v.gu = -1;
         if (i < n_kept) {
             const uint2 geo = a.sgeo[i];
             if (!(geo.x & 0x8000u)) v = vis_hits(a, geo);                      // merged duplicates have no hits of their own
         }
-        mine += v.n;
-#if IMAGER_AGGREGATE
-        const int n_max = __reduce_max_sync(0xffffffffu, v.n);
-        for (int t = 0; t < n_max; ++t) {
-            const bool on = t < v.n;
-            const int ty = on ? t / v.nsx : 0;
-            const long long cell = on ? v.cell0 + (int64_t)ty * g.strips_per_row + (t - ty * v.nsx) : -1ll - lane;
-            const unsigned peers = __match_any_sync(0xffffffffu, cell);         // lanes that meet the same (gu, strip)
-            if (on && lane == __ffs(peers) - 1) atomicAdd(hits + cell, __popc(peers));
+        mine_total += v.n;
+        const bool valid = v.n > 0;
+        unsigned pending = __ballot_sync(0xffffffffu, valid);
+        while (pending) {
+            const HitWindow win = next_window(v, valid, pending);
+            const bool mine = (win.group >> lane) & 1u;
+            const int64_t cell0 = (int64_t)win.gu * g.n_strips;
+            if (win.w * win.h <= kWindowMax) {
+                int cnt0 = 0, cnt1 = 0, t = 0;
+                for (int Y = win.y_lo; Y < win.y_lo + win.h; ++Y)
+                    for (int X = win.x_lo; X < win.x_lo + win.w; ++X, ++t) {
+                        const bool in = mine && (unsigned)(X - v.sx0) < (unsigned)v.nsx && (unsigned)(Y - v.sy0) < (unsigned)v.nsy;
+                        const int c = __popc(__ballot_sync(0xffffffffu, in));
+                        if (lane == (t & 31)) {
+                            if (t < 32) cnt0 = c; else cnt1 = c;
+                        }
+                    }
+                if (cnt0) {
+                    const int ty = lane / win.w;
+                    atomicAdd(hits + cell0 + (int64_t)(win.y_lo + ty) * g.strips_per_row + win.x_lo + (lane - ty * win.w), cnt0);
+                }
+                if (cnt1) {
+                    const int t1 = lane + 32, ty = t1 / win.w;
+                    atomicAdd(hits + cell0 + (int64_t)(win.y_lo + ty) * g.strips_per_row + win.x_lo + (t1 - ty * win.w), cnt1);
+                }
+            } else if (mine) {                 // a group that straddles the end of a tile row: every lane on its own
+                for (int ty = 0; ty < v.nsy; ++ty)
+                    for (int tx = 0; tx < v.nsx; ++tx)
+                        atomicAdd(hits + cell0 + (int64_t)(v.sy0 + ty) * g.strips_per_row + v.sx0 + tx, 1);
+            }
+            pending &= ~win.group;
         }
-#else
-        for (int t = 0; t < v.n; ++t) {
-            const int ty = t / v.nsx;
-            atomicAdd(hits + v.cell0 + (int64_t)ty * g.strips_per_row + (t - ty * v.nsx), 1);
-        }
-#endif
     }
-    mine = __reduce_add_sync(0xffffffffu, mine);       // < 2^31: a thread sees at most 2^31 / gridDim visibilities x 162 strips
-    if (lane == 0 && mine) atomicAdd(total, (unsigned long long)mine);
+    mine_total = __reduce_add_sync(0xffffffffu, mine_total);   // < 2^31: a thread sees at most 2^31 / gridDim visibilities x 162 strips
+    if (lane == 0 && mine_total) atomicAdd(total, (unsigned long long)mine_total);
 }
 
 // items[cell] = ceil(hits[cell] / kItemHits); entry n_cells (the terminator of the exclusive scans) is 0 in both
@@ -316,8 +352,17 @@ __global__ void items_from_hits_kernel(int64_t n_cells, const int32_t* __restric
         items[c] = c < n_cells ? (hits[c] + kItemHits - 1) / kItemHits : 0;
 }
 
-// Unsorted hit records, visibility-centric: the same enumeration as count_hits_kernel; a hit takes the next free place
-// of its cell's range (hit_start[cell] + cursor[cell]++).
+// Unsorted hit records, visibility-centric: the same walk as count_hits_kernel.  Per window strip one lane reserves
+// the places of the warp's hits with ONE atomic on the cell's cursor; a lane's hit takes place hit_start[cell] + that
+// base + its rank among the lanes that meet the strip.
+__device__ __forceinline__ void emit_one(const VisHits& v, int i, int X, int Y, int pitch, int slice_taps, int group_slices,
+                                         int64_t pos, uint2* __restrict__ hit_tmp) {
+    const int dx0 = X * kStripW - v.x0, dy0 = Y * kStripH - v.y0;          // taps of the strip origin
+    const uint32_t ctrl = hit_ctrl(dx0, dy0, v.S, v.subl, group_slices);
+    const int tapoff = v.subl * slice_taps + (dy0 + kPadY) * pitch + dx0 + kPadX;
+    hit_tmp[pos] = make_uint2((uint32_t)i, (uint32_t)(tapoff + (int)kTapBias) | (ctrl << 24));
+}
+
 __global__ void emit_hits_kernel(const PlanArgs a, const int32_t* __restrict__ counters, const int32_t* __restrict__ hit_start,
                                  int32_t* __restrict__ cursor, uint2* __restrict__ hit_tmp) {
     const Geometry& g = a.g;
@@ -328,6 +373,7 @@ __global__ void emit_hits_kernel(const PlanArgs a, const int32_t* __restrict__ c
         const int i = i0 + lane;
         VisHits v;
         v.n = 0;
+        v.gu = -1;
         int pitch = 0, slice_taps = 0, group_slices = 1;
         uint2 geo = make_uint2(0x8000u, 0u);
         if (i < n_kept) geo = a.sgeo[i];
@@ -338,51 +384,51 @@ __global__ void emit_hits_kernel(const PlanArgs a, const int32_t* __restrict__ c
             slice_taps = sp.rows * sp.pitch;
             group_slices = sp.group_slices;
         }
-#if IMAGER_AGGREGATE
-        const int n_max = __reduce_max_sync(0xffffffffu, v.n);
-#else
-        const int n_max = v.n;
-#endif
-        // four strips at a time: their cursor atomics (which return a value) are in flight together
-        for (int t0 = 0; t0 < n_max; t0 += 4) {
-            long long cell[4];
-            unsigned peers[4];
-            int base[4], start[4];
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const int t = t0 + q;
-                const bool on = t < v.n;
-                const int ty = on ? t / v.nsx : 0, tx = t - ty * v.nsx;
-                cell[q] = on ? v.cell0 + (int64_t)ty * g.strips_per_row + tx : -1ll - lane;
-                base[q] = start[q] = 0;
-                peers[q] = 1u << lane;
-                if (t < n_max) {                                            // warp-uniform
-#if IMAGER_AGGREGATE
-                    peers[q] = __match_any_sync(0xffffffffu, cell[q]);
-                    if (on && lane == __ffs(peers[q]) - 1) base[q] = atomicAdd(cursor + cell[q], __popc(peers[q]));
-#else
-                    if (on) base[q] = atomicAdd(cursor + cell[q], 1);
-#endif
-                    if (on) start[q] = hit_start[cell[q]];
+        const bool valid = v.n > 0;
+        unsigned pending = __ballot_sync(0xffffffffu, valid);
+        while (pending) {
+            const HitWindow win = next_window(v, valid, pending);
+            const bool mine = (win.group >> lane) & 1u;
+            const int64_t cell0 = (int64_t)win.gu * g.n_strips;
+            if (win.w * win.h <= kWindowMax) {
+                int cnt0 = 0, cnt1 = 0, t = 0;
+                for (int Y = win.y_lo; Y < win.y_lo + win.h; ++Y)
+                    for (int X = win.x_lo; X < win.x_lo + win.w; ++X, ++t) {
+                        const bool in = mine && (unsigned)(X - v.sx0) < (unsigned)v.nsx && (unsigned)(Y - v.sy0) < (unsigned)v.nsy;
+                        const int c = __popc(__ballot_sync(0xffffffffu, in));
+                        if (lane == (t & 31)) {
+                            if (t < 32) cnt0 = c; else cnt1 = c;
+                        }
+                    }
+                int pos0 = 0, pos1 = 0;                                       // first place of window strip `lane` / `lane + 32`
+                if (cnt0) {
+                    const int ty = lane / win.w;
+                    const int64_t cell = cell0 + (int64_t)(win.y_lo + ty) * g.strips_per_row + win.x_lo + (lane - ty * win.w);
+                    pos0 = hit_start[cell] + atomicAdd(cursor + cell, cnt0);
                 }
-            }
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const int t = t0 + q;
-                if (t >= n_max) break;                                      // warp-uniform
-#if IMAGER_AGGREGATE
-                const int pos = __shfl_sync(0xffffffffu, base[q], __ffs(peers[q]) - 1) + __popc(peers[q] & lt_mask);
-#else
-                const int pos = base[q];
-#endif
-                if (t < v.n) {
-                    const int ty = t / v.nsx, tx = t - ty * v.nsx;
-                    const int dx0 = (v.sx0 + tx) * kStripW - v.x0, dy0 = (v.sy0 + ty) * kStripH - v.y0;   // taps of the strip origin
-                    const uint32_t ctrl = hit_ctrl(dx0, dy0, v.S, v.subl, group_slices);
-                    const int tapoff = v.subl * slice_taps + (dy0 + kPadY) * pitch + dx0 + kPadX;
-                    hit_tmp[(int64_t)start[q] + pos] = make_uint2((uint32_t)i, (uint32_t)(tapoff + (int)kTapBias) | (ctrl << 24));
+                if (cnt1) {
+                    const int t1 = lane + 32, ty = t1 / win.w;
+                    const int64_t cell = cell0 + (int64_t)(win.y_lo + ty) * g.strips_per_row + win.x_lo + (t1 - ty * win.w);
+                    pos1 = hit_start[cell] + atomicAdd(cursor + cell, cnt1);
                 }
+                t = 0;
+                for (int Y = win.y_lo; Y < win.y_lo + win.h; ++Y)
+                    for (int X = win.x_lo; X < win.x_lo + win.w; ++X, ++t) {
+                        const bool in = mine && (unsigned)(X - v.sx0) < (unsigned)v.nsx && (unsigned)(Y - v.sy0) < (unsigned)v.nsy;
+                        const unsigned b = __ballot_sync(0xffffffffu, in);
+                        if (b == 0u) continue;                                      // warp-uniform
+                        const int base = __shfl_sync(0xffffffffu, t < 32 ? pos0 : pos1, t & 31);
+                        if (in) emit_one(v, i, X, Y, pitch, slice_taps, group_slices, (int64_t)base + __popc(b & lt_mask), hit_tmp);
+                    }
+            } else if (mine) {
+                for (int ty = 0; ty < v.nsy; ++ty)
+                    for (int tx = 0; tx < v.nsx; ++tx) {
+                        const int64_t cell = cell0 + (int64_t)(v.sy0 + ty) * g.strips_per_row + v.sx0 + tx;
+                        emit_one(v, i, v.sx0 + tx, v.sy0 + ty, pitch, slice_taps, group_slices,
+                                 (int64_t)hit_start[cell] + atomicAdd(cursor + cell, 1), hit_tmp);
+                    }
             }
+            pending &= ~win.group;
         }
     }
 }
