@@ -55,7 +55,10 @@ constexpr int kStageBytes = kWarps * 32 * 16;         // per-warp hit descriptor
 constexpr int kStageSlots = 40;                       // gridding: 32 descriptors + the one read past a batch's end
 constexpr int kGridStageBytes = (kGridThreads / 32) * kStageSlots * 16;
 constexpr int kMaxSmem = 227 * 1024;
-constexpr int kRedSlots = 8;                           // degridding: hits per transposed reduction
+#ifndef IMAGER_RED_SLOTS
+#define IMAGER_RED_SLOTS 16
+#endif
+constexpr int kRedSlots = IMAGER_RED_SLOTS;            // degridding: hits per transposed reduction (8, 16 or 32)
 constexpr int kRedBytes = kWarps * kRedSlots * 32 * 8;
 constexpr int kTableBudget = kMaxSmem - (kStageBytes + kRedBytes > kGridStageBytes ? kStageBytes + kRedBytes : kGridStageBytes) - 1024;   // 1 KB: static
 constexpr int64_t kMaxPlanCells = (int64_t)1 << 30;   // (geometry unit, strip) pairs: 12 bytes of planner state each
@@ -942,20 +945,23 @@ degrid_tiled_kernel(const TiledArgs a, const float2* __restrict__ grid, float2* 
                         // transposed reduction of hits [h0, h): lane = slot + 8 * quarter sums columns 8 q .. 8 q + 7
                         const int h0 = (h - 1) & ~(kRedSlots - 1);
                         __syncwarp();
-                        const int slot = lane & (kRedSlots - 1), q = lane >> 3;
+                        // lane = slot + kRedSlots * part sums the kRedCols columns of its part
+                        constexpr int kRedParts = 32 / kRedSlots, kRedCols = 32 / kRedParts;
+                        const int slot = lane & (kRedSlots - 1), q = lane / kRedSlots;
                         float2 acc = make_float2(0.f, 0.f);
                         if (h0 + slot < h) {
 #pragma unroll
-                            for (int k = 0; k < 8; ++k) {
-                                const float2 v = lds64(red_base + (uint32_t)((slot * 32 + 8 * q + ((k + slot) & 7)) * 8));
+                            for (int k = 0; k < kRedCols; ++k) {
+                                const float2 v = lds64(red_base + (uint32_t)((slot * 32 + kRedCols * q + ((k + slot) & (kRedCols - 1))) * 8));
                                 acc.x += v.x;
                                 acc.y += v.y;
                             }
                         }
-                        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 8);
-                        acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 8);
-                        acc.x += __shfl_xor_sync(0xffffffffu, acc.x, 16);
-                        acc.y += __shfl_xor_sync(0xffffffffu, acc.y, 16);
+#pragma unroll
+                        for (int d = kRedSlots; d < 32; d <<= 1) {
+                            acc.x += __shfl_xor_sync(0xffffffffu, acc.x, d);
+                            acc.y += __shfl_xor_sync(0xffffffffu, acc.y, d);
+                        }
                         if (lane < kRedSlots && h0 + lane < h) {
                             const uint32_t idx = stage[h0 + lane].y;
                             atomicAdd(&ssum[(int64_t)idx * NC + c_corr], acc);
