@@ -254,6 +254,15 @@ int imager_index_stats(imager_plan* plan, int64_t out[8], void* cuda_stream);
  * (host-side counter, no synchronisation); negative status on a NULL plan. */
 int imager_last_launch_count(imager_plan* plan);
 
+/* Self-checks of a CHECKED build (libimager_checked.so, compiled with -DIMAGER_CHECKED=1: every index the planner and the
+ * tiled kernels form -- hit-record places, visibility indices, shared-memory tap addresses, strips, work items -- is
+ * tested against its bounds on the device and violations are counted instead of being dereferenced blindly; the pool's
+ * compute-sanitizer is closed).  out[k], k = 0..15: violations of check k since the library was
+ * loaded (k: 0 hit place, 1 visibility index of a hit, 2 tap address, 3 strip, 4 item range, 5 block range, 6 hash
+ * table, 7 window strip).  Returns 1 for a checked build, 0 for the normal build (out is zeroed), < 0 on error.
+ * Synchronises the device. */
+int imager_debug_violations(int64_t out[16]);
+
 /* Thread-local message of the last failing call on this thread ("" if none); valid until the next call. */
 const char* imager_last_error(void);
 

@@ -13,7 +13,7 @@ from ctypes import (POINTER, Structure, byref, c_char_p, c_double, c_float, c_in
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libimager.so")
+LIB_PATH = os.environ.get("IMAGER_LIBRARY") or os.path.join(_HERE, "libimager.so")   # IMAGER_LIBRARY: e.g. the checked build
 
 MODE_DELTA, MODE_PSWF, MODE_WPROJ, MODE_AWPROJ_ADJOINT, MODE_AWPROJ_PAPER, MODE_MOSAIC_PB, MODE_USER = range(7)
 REUSE_INDEX = 1
@@ -24,7 +24,7 @@ EXPORTS = ("imager_plan_create", "imager_index", "imager_grid", "imager_degrid",
            "imager_grid_image_transform", "imager_mosaic_correct", "imager_debug_index", "imager_debug_kernels", "imager_plan_info",
            "imager_index_stats", "imager_hogbom", "imager_clean", "imager_reproject", "imager_mosaic_grid",
            "imager_mosaic_degrid",
-           "imager_last_launch_count", "imager_last_error")
+           "imager_last_launch_count", "imager_debug_violations", "imager_last_error")
 
 
 class ImagerError(RuntimeError):
@@ -80,6 +80,7 @@ def load_library() -> ctypes.CDLL:
     lib.imager_clean.argtypes = [c_void_p, c_int64, c_void_p, c_void_p, c_void_p, c_void_p, POINTER(ImagerCleanParams), c_void_p,
                                  c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
     lib.imager_last_launch_count.argtypes = [c_void_p]
+    lib.imager_debug_violations.argtypes = [POINTER(c_int64)]
     _lib = lib
     return lib
 

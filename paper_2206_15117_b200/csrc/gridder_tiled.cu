@@ -28,6 +28,19 @@
 
 namespace imager {
 
+// ---- checked build (-DIMAGER_CHECKED=1 -> libimager_checked.so): every index formed below is tested against its
+// bounds and violations are counted per check (imager_debug_violations) instead of being dereferenced blindly ----
+#ifndef IMAGER_CHECKED
+#define IMAGER_CHECKED 0
+#endif
+__device__ unsigned long long g_violations[16];
+#if IMAGER_CHECKED
+#define IMAGER_CHECK(k, cond) ((cond) ? true : (atomicAdd(&g_violations[k], 1ull), false))
+#else
+#define IMAGER_CHECK(k, cond) (true)
+#endif
+enum { kChkHitPlace = 0, kChkVisIndex = 1, kChkTapAddr = 2, kChkStrip = 3, kChkItem = 4, kChkBlock = 5, kChkHash = 6, kChkWindow = 7 };
+
 constexpr int kLaneW = 8, kLaneH = 4;                 // lane block
 constexpr int kNX = 2, kNY = 8;                       // replications: strip = 16 x 32 cells
 constexpr int kStripW = kLaneW * kNX, kStripH = kLaneH * kNY;
@@ -147,15 +160,17 @@ __global__ void __launch_bounds__(kDedupeThreads, 2) sorted_geo_dedupe_kernel(co
             if (i >= c1) continue;
             const unsigned long long key = ((unsigned long long)geo[j].y << 32) | geo[j].x;
             uint32_t h = (uint32_t)((key * 0x9E3779B97F4A7C15ull) >> 51) & (kDedupeSlots - 1);
-            for (;;) {
+            for (int probes = 0;; ++probes) {
                 const unsigned long long old = pass == 0 ? atomicCAS(&s_key[h], ~0ull, key) : s_key[h];
                 if (old == key || (pass == 0 && old == ~0ull)) break;
+                if (!IMAGER_CHECK(kChkHash, probes < kDedupeSlots)) break;      // load factor <= 0.5: cannot happen
                 h = (h + 1) & (kDedupeSlots - 1);
             }
             if (pass == 0) {
                 atomicMin(&s_idx[h], i);
             } else {
                 const int r = s_idx[h];
+                IMAGER_CHECK(kChkHash, r >= c0 && r <= i);
                 rep[i] = r;
                 sgeo[i] = make_uint2(geo[j].x | (r != i ? kMergedFlag : 0u), geo[j].y);
             }
@@ -224,6 +239,7 @@ struct PlanArgs {
     const int32_t* gu_set;
     const int32_t* set_support;
     const uint2* sgeo;
+    int64_t cap_hits;          // capacity of the hit-record arrays (checked build)
 };
 
 // ctrl byte of a candidate against a strip, or 0 if it is no hit (a hit always has bit 6 or 7 set)
@@ -294,6 +310,7 @@ __device__ __forceinline__ HitWindow next_window(const VisHits& v, bool valid, u
     win.y_lo = __reduce_min_sync(0xffffffffu, mine ? v.sy0 : 0x7fffffff);
     win.w = __reduce_max_sync(0xffffffffu, mine ? v.sx0 + v.nsx : 0) - win.x_lo;
     win.h = __reduce_max_sync(0xffffffffu, mine ? v.sy0 + v.nsy : 0) - win.y_lo;
+    IMAGER_CHECK(kChkWindow, win.x_lo >= 0 && win.y_lo >= 0 && win.w >= 1 && win.h >= 1);
     return win;
 }
 
@@ -319,6 +336,8 @@ __global__ void count_hits_kernel(const PlanArgs a, const int32_t* __restrict__ 
             const HitWindow win = next_window(v, valid, pending);
             const bool mine = (win.group >> lane) & 1u;
             const int64_t cell0 = (int64_t)win.gu * g.n_strips;
+            IMAGER_CHECK(kChkWindow, win.gu >= 0 && win.gu < g.n_gu && win.x_lo + win.w <= g.strips_per_row &&
+                                         (win.y_lo + win.h) * g.strips_per_row <= g.n_strips);
             if (win.w * win.h <= kWindowMax) {
                 int cnt0 = 0, cnt1 = 0, t = 0;
                 for (int Y = win.y_lo; Y < win.y_lo + win.h; ++Y)
@@ -359,10 +378,11 @@ __global__ void items_from_hits_kernel(int64_t n_cells, const int32_t* __restric
 // the places of the warp's hits with ONE atomic on the cell's cursor; a lane's hit takes place hit_start[cell] + that
 // base + its rank among the lanes that meet the strip.
 __device__ __forceinline__ void emit_one(const VisHits& v, int i, int X, int Y, int pitch, int slice_taps, int group_slices,
-                                         int64_t pos, uint2* __restrict__ hit_tmp) {
+                                         int64_t pos, uint2* __restrict__ hit_tmp, const int32_t* __restrict__ range) {
     const int dx0 = X * kStripW - v.x0, dy0 = Y * kStripH - v.y0;          // taps of the strip origin
     const uint32_t ctrl = hit_ctrl(dx0, dy0, v.S, v.subl, group_slices);
     const int tapoff = v.subl * slice_taps + (dy0 + kPadY) * pitch + dx0 + kPadX;
+    if (!IMAGER_CHECK(kChkHitPlace, ctrl != 0u && pos >= range[0] && pos < range[1])) return;   // range = hit_start + cell
     hit_tmp[pos] = make_uint2((uint32_t)i, (uint32_t)(tapoff + (int)kTapBias) | (ctrl << 24));
 }
 
@@ -393,6 +413,8 @@ __global__ void emit_hits_kernel(const PlanArgs a, const int32_t* __restrict__ c
             const HitWindow win = next_window(v, valid, pending);
             const bool mine = (win.group >> lane) & 1u;
             const int64_t cell0 = (int64_t)win.gu * g.n_strips;
+            IMAGER_CHECK(kChkWindow, win.gu >= 0 && win.gu < g.n_gu && win.x_lo + win.w <= g.strips_per_row &&
+                                         (win.y_lo + win.h) * g.strips_per_row <= g.n_strips);
             if (win.w * win.h <= kWindowMax) {
                 int cnt0 = 0, cnt1 = 0, t = 0;
                 for (int Y = win.y_lo; Y < win.y_lo + win.h; ++Y)
@@ -421,14 +443,15 @@ __global__ void emit_hits_kernel(const PlanArgs a, const int32_t* __restrict__ c
                         const unsigned b = __ballot_sync(0xffffffffu, in);
                         if (b == 0u) continue;                                      // warp-uniform
                         const int base = __shfl_sync(0xffffffffu, t < 32 ? pos0 : pos1, t & 31);
-                        if (in) emit_one(v, i, X, Y, pitch, slice_taps, group_slices, (int64_t)base + __popc(b & lt_mask), hit_tmp);
+                        if (in) emit_one(v, i, X, Y, pitch, slice_taps, group_slices, (int64_t)base + __popc(b & lt_mask), hit_tmp,
+                                         hit_start + cell0 + (int64_t)Y * g.strips_per_row + X);
                     }
             } else if (mine) {
                 for (int ty = 0; ty < v.nsy; ++ty)
                     for (int tx = 0; tx < v.nsx; ++tx) {
                         const int64_t cell = cell0 + (int64_t)(v.sy0 + ty) * g.strips_per_row + v.sx0 + tx;
                         emit_one(v, i, v.sx0 + tx, v.sy0 + ty, pitch, slice_taps, group_slices,
-                                 (int64_t)hit_start[cell] + atomicAdd(cursor + cell, 1), hit_tmp);
+                                 (int64_t)hit_start[cell] + atomicAdd(cursor + cell, 1), hit_tmp, hit_start + cell);
                     }
             }
             pending &= ~win.group;
@@ -586,7 +609,29 @@ struct TiledArgs {
     const int32_t* set_support;
     const SetPlan* set_plan;
     const int32_t* gu_set;
+    int64_t n_hits;             // totals of the plan (checked build)
+    int32_t n_items;
 };
+
+// checked build: a staged hit must stay inside the resident table group, name a kept visibility and a strip of the grid
+__device__ __forceinline__ bool check_hit(const TiledArgs& a, const SetPlan& sp, const Item& it, bool live, uint2 rec) {
+#if IMAGER_CHECKED
+    bool ok = IMAGER_CHECK(kChkStrip, it.strip >= 0 && it.strip < a.g.n_strips && it.hit_begin >= 0 &&
+                                          (int64_t)it.hit_begin + it.hit_count <= a.n_hits);
+    if (live) {
+        const uint32_t ctrl = rec.y >> 24;
+        const int tapoff = (int)(rec.y & 0xffffffu) - (int)kTapBias;
+        const int jl = (int)(ctrl & 7u), jh1 = (int)((ctrl >> 3) & 7u);
+        const int lo = tapoff + jl * kLaneH * sp.pitch + ((ctrl & 0x40u) ? 0 : kLaneW);
+        const int hi = tapoff + (jh1 * kLaneH + kLaneH - 1) * sp.pitch + ((ctrl & 0x80u) ? kStripW - 1 : kLaneW - 1);
+        ok = IMAGER_CHECK(kChkTapAddr, (ctrl >> 6) != 0u && jl <= jh1 && lo >= 0 && hi < sp.group_slices * sp.rows * sp.pitch) && ok;
+        ok = IMAGER_CHECK(kChkVisIndex, (int)rec.x >= 0 && (int)rec.x < a.queue[-8]) && ok;     // queue = counters + 8; counters[0] = n_kept
+    }
+    return ok;
+#else
+    return true;
+#endif
+}
 
 // copy one slice group of element sc of kernel set `kset` into shared memory: [slice][row -3 .. S+2][col -7 ..], zero padded
 __device__ void load_table_group(const TiledArgs& a, int kset, int group, int sc, const SetPlan sp, int S, float2* tab_s) {
@@ -727,6 +772,8 @@ grid_tiled_kernel(const TiledArgs a, const float2* __restrict__ sval, float2* __
         if (s_block >= n_blocks) break;
         const Block blk = a.blocks[s_block < n_front ? s_block : a.cap_blocks - 1 - (s_block - n_front)];
         if (blk.item_count == 0) continue;
+        if (!IMAGER_CHECK(kChkBlock, n_blocks <= a.cap_blocks && blk.gu >= 0 && blk.gu < g.n_gu && blk.sc >= 0 && blk.sc < g.n_pol * g.n_corr &&
+                                         blk.item_begin >= 0 && blk.item_begin + blk.item_count <= a.n_items)) continue;
         const int kset = a.gu_set[blk.gu];
         const SetPlan sp = a.set_plan[kset];
         const int S = a.set_support[kset];
@@ -763,6 +810,7 @@ grid_tiled_kernel(const TiledArgs a, const float2* __restrict__ sval, float2* __
             if (lane < it.hit_count) val = sval[(int64_t)rec.x * NC + c_corr];
             for (int b0 = 0; b0 < it.hit_count; b0 += 32) {
                 const int n = min(32, it.hit_count - b0);
+                if (!check_hit(a, sp, it, lane < n, rec)) rec = make_uint2(0u, kTapBias | (0x40u << 24));   // checked build: a harmless hit
                 const uint32_t my_ctrl = lane < n ? rec.y >> 24 : 0x40u;
                 const uint32_t my_variant = ctrl_variant(my_ctrl);
                 stage[lane] = make_uint4(__float_as_uint(val.x), __float_as_uint(val.y),
@@ -891,6 +939,8 @@ degrid_tiled_kernel(const TiledArgs a, const float2* __restrict__ grid, float2* 
         if (s_block >= n_blocks) break;
         const Block blk = a.blocks[s_block < n_front ? s_block : a.cap_blocks - 1 - (s_block - n_front)];
         if (blk.item_count == 0) continue;
+        if (!IMAGER_CHECK(kChkBlock, n_blocks <= a.cap_blocks && blk.gu >= 0 && blk.gu < g.n_gu && blk.sc >= 0 && blk.sc < g.n_pol * g.n_corr &&
+                                         blk.item_begin >= 0 && blk.item_begin + blk.item_count <= a.n_items)) continue;
         const int kset = a.gu_set[blk.gu];
         const SetPlan sp = a.set_plan[kset];
         const int S = a.set_support[kset];
@@ -925,6 +975,7 @@ degrid_tiled_kernel(const TiledArgs a, const float2* __restrict__ grid, float2* 
             if (lane + 32 < it.hit_count) rec1 = a.hit_rec[it.hit_begin + 32 + lane];
             for (int b0 = 0; b0 < it.hit_count; b0 += 32) {
                 const int n = min(32, it.hit_count - b0);
+                if (!check_hit(a, sp, it, lane < n, rec)) rec = make_uint2(0u, kTapBias | (0x40u << 24));   // checked build: a harmless hit
                 const uint32_t my_ctrl = lane < n ? rec.y >> 24 : 0x40u;
                 const uint32_t my_variant = ctrl_variant(my_ctrl);
                 stage[lane] = make_uint2(tab_addr + (uint32_t)(((int)(rec.y & 0xffffffu) - (int)kTapBias) * 8), rec.x);
@@ -1174,6 +1225,7 @@ static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
     pa.gu_set = st->d_gu_set;
     pa.set_support = pl->d_set_support;
     pa.sgeo = st->d_sgeo;
+    pa.cap_hits = 0;
     IMAGER_CUDA(cudaMemsetAsync(st->d_hits, 0, (n_cells + 1) * sizeof(int32_t), stream));
     IMAGER_CUDA(cudaMemsetAsync(st->d_total, 0, sizeof(unsigned long long), stream));
     count_hits_kernel<<<8 * kNumSMs, 256, 0, stream>>>(pa, pl->d_counters, st->d_hits, st->d_total);
@@ -1240,6 +1292,8 @@ static void fill_args(imager_plan* pl, TiledState* st, TiledArgs& a, const float
     a.set_support = pl->d_set_support;
     a.set_plan = st->d_plan;
     a.gu_set = st->d_gu_set;
+    a.n_hits = st->h_totals ? st->h_totals[0] : 0;
+    a.n_items = st->h_totals ? *reinterpret_cast<int32_t*>(&st->h_totals[1]) : 0;
 }
 
 // imager_index_stats: sums over the sorted kept visibilities.  out: [0] sum S^2 of all kept, [1] sum S^2 of those that
@@ -1356,3 +1410,13 @@ int launch_degrid_tiled(imager_plan* pl, int64_t nvis, const float2* grid, float
 }
 
 }  // namespace imager
+
+extern "C" int imager_debug_violations(int64_t out[16]) {
+    if (!out) return IMAGER_ERR_INVALID_ARG;
+    unsigned long long h[16] = {0};
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = cudaMemcpyFromSymbol(h, imager::g_violations, sizeof(h));
+    if (e != cudaSuccess) return imager::cuda_fail(e, "imager_debug_violations");
+    for (int k = 0; k < 16; ++k) out[k] = (int64_t)h[k];
+    return IMAGER_CHECKED ? 1 : 0;
+}
