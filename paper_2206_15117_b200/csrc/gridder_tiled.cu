@@ -417,12 +417,19 @@ __global__ void emit_hits_kernel(const PlanArgs a, const int32_t* __restrict__ c
                                          (win.y_lo + win.h) * g.strips_per_row <= g.n_strips);
             if (win.w * win.h <= kWindowMax) {
                 int cnt0 = 0, cnt1 = 0, t = 0;
+                unsigned bal0 = 0u, bal1 = 0u;                               // lane t: the lanes that meet window strip t / t + 32
                 for (int Y = win.y_lo; Y < win.y_lo + win.h; ++Y)
                     for (int X = win.x_lo; X < win.x_lo + win.w; ++X, ++t) {
                         const bool in = mine && (unsigned)(X - v.sx0) < (unsigned)v.nsx && (unsigned)(Y - v.sy0) < (unsigned)v.nsy;
-                        const int c = __popc(__ballot_sync(0xffffffffu, in));
+                        const unsigned b = __ballot_sync(0xffffffffu, in);
                         if (lane == (t & 31)) {
-                            if (t < 32) cnt0 = c; else cnt1 = c;
+                            if (t < 32) {
+                                cnt0 = __popc(b);
+                                bal0 = b;
+                            } else {
+                                cnt1 = __popc(b);
+                                bal1 = b;
+                            }
                         }
                     }
                 int pos0 = 0, pos1 = 0;                                       // first place of window strip `lane` / `lane + 32`
@@ -436,16 +443,32 @@ __global__ void emit_hits_kernel(const PlanArgs a, const int32_t* __restrict__ c
                     const int64_t cell = cell0 + (int64_t)(win.y_lo + ty) * g.strips_per_row + win.x_lo + (t1 - ty * win.w);
                     pos1 = hit_start[cell] + atomicAdd(cursor + cell, cnt1);
                 }
-                t = 0;
-                for (int Y = win.y_lo; Y < win.y_lo + win.h; ++Y)
-                    for (int X = win.x_lo; X < win.x_lo + win.w; ++X, ++t) {
-                        const bool in = mine && (unsigned)(X - v.sx0) < (unsigned)v.nsx && (unsigned)(Y - v.sy0) < (unsigned)v.nsy;
-                        const unsigned b = __ballot_sync(0xffffffffu, in);
-                        if (b == 0u) continue;                                      // warp-uniform
-                        const int base = __shfl_sync(0xffffffffu, t < 32 ? pos0 : pos1, t & 31);
-                        if (in) emit_one(v, i, X, Y, pitch, slice_taps, group_slices, (int64_t)base + __popc(b & lt_mask), hit_tmp,
-                                         hit_start + cell0 + (int64_t)Y * g.strips_per_row + X);
+                // every lane walks its own strips: place = the strip's base + this lane's rank among the lanes that meet it
+                const bool big = win.w * win.h > 32;                           // warp-uniform
+                const int n_own = mine ? v.n : 0;
+                const int n_max = __reduce_max_sync(0xffffffffu, n_own);
+                int tx = 0, ty = 0;
+                for (int q = 0; q < n_max; ++q) {
+                    const bool on = q < n_own;
+                    const int X = v.sx0 + tx, Y = v.sy0 + ty;
+                    const int wi = on ? (Y - win.y_lo) * win.w + (X - win.x_lo) : 0;
+                    int base = __shfl_sync(0xffffffffu, pos0, wi & 31);
+                    unsigned b = __shfl_sync(0xffffffffu, bal0, wi & 31);
+                    if (big) {
+                        const int base1 = __shfl_sync(0xffffffffu, pos1, wi & 31);
+                        const unsigned b1 = __shfl_sync(0xffffffffu, bal1, wi & 31);
+                        if (wi >= 32) {
+                            base = base1;
+                            b = b1;
+                        }
                     }
+                    if (on) emit_one(v, i, X, Y, pitch, slice_taps, group_slices, (int64_t)base + __popc(b & lt_mask), hit_tmp,
+                                     hit_start + cell0 + (int64_t)Y * g.strips_per_row + X);
+                    if (++tx == v.nsx) {
+                        tx = 0;
+                        ++ty;
+                    }
+                }
             } else if (mine) {
                 for (int ty = 0; ty < v.nsy; ++ty)
                     for (int tx = 0; tx < v.nsx; ++tx) {
@@ -480,7 +503,7 @@ __global__ void make_items_kernel(const Geometry g, const int32_t* __restrict__ 
 #define IMAGER_SORT_ITEMS 2
 #endif
 constexpr int kSortSpan = IMAGER_SORT_ITEMS * kItemHits;
-__global__ void __launch_bounds__(256) sort_items_kernel(int n_items, const Item* __restrict__ item_rec,
+__global__ void __launch_bounds__(256, 4) sort_items_kernel(int n_items, const Item* __restrict__ item_rec,
                                                          const uint2* __restrict__ hit_tmp, uint2* __restrict__ hit_rec) {
     __shared__ int32_t s_bin[8][128];
     const int item = (int)(((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5);

@@ -17,9 +17,9 @@
 
 namespace imager {
 
-__device__ __forceinline__ long long floor_div(long long a, long long b) {
-    long long q = a / b;
-    return (a % b != 0 && ((a < 0) != (b < 0))) ? q - 1 : q;
+__device__ __forceinline__ int floor_div32(int a, int b) {      // b > 0
+    const int q = a / b;
+    return (a - q * b < 0) ? q - 1 : q;
 }
 
 __global__ void index_kernel(int64_t nvis, const float* __restrict__ uvw, const int32_t* __restrict__ a_index,
@@ -44,28 +44,29 @@ __global__ void index_kernel(int64_t nvis, const float* __restrict__ uvw, const 
         key[k] = key_drop;
         return;
     }
-    const long long qx = __double2ll_rn(su);
-    const long long qy = __double2ll_rn(sv);
+    // |su|, |sv| < 2^30 from here on: 32-bit integer arithmetic gives the same values as the 64-bit definition
+    const int qx = __double2int_rn(su), qy = __double2int_rn(sv);
     const int half_o = O / 2;
-    const long long ix = floor_div(qx + half_o, O), iy = floor_div(qy + half_o, O);
-    const int ox = (int)(qx - ix * O), oy = (int)(qy - iy * O);
-    const long long gx = ix + N / 2, gy = iy + N / 2;
-    long long p = __double2ll_rn(__dmul_rn(fabs((double)w), w_scale));
-    if (p > P - 1) p = P - 1;
-    const int sp = (w < 0.f) ? -(int)p : (int)p;
+    const int ix = floor_div32(qx + half_o, O), iy = floor_div32(qy + half_o, O);
+    const int ox = qx - ix * O, oy = qy - iy * O;
+    const int gx = ix + N / 2, gy = iy + N / 2;
+    // p = min(P - 1, rint(|w| w_scale)): the comparison is made in double so that huge |w| clamps instead of wrapping
+    const double sw = __dmul_rn(fabs((double)w), w_scale);
+    const int p = sw >= (double)(P - 1) ? P - 1 : __double2int_rn(sw);
+    const int sp = (w < 0.f) ? -p : p;
     const int kset = a * (2 * P - 1) + sp + P - 1;
     const int S = plane_support[p], h_lo = S / 2, h_hi = S - 1 - h_lo;
     const bool drop = (gx - h_lo < 0) || (gx + h_hi >= N) || (gy - h_lo < 0) || (gy + h_hi >= N);
     imager_record r;
-    r.gx = (int32_t)gx;
-    r.gy = (int32_t)gy;
+    r.gx = gx;
+    r.gy = gy;
     r.sub = (uint32_t)(ox + half_o) | ((uint32_t)(oy + half_o) << 8) | ((uint32_t)drop << 16);
     r.kset = kset;
     rec[k] = r;
     uint32_t kk = key_drop;
-    if (!drop)
-        kk = (uint32_t)((((long long)kset * nt + gy / kBucketTile) * nt + gx / kBucketTile) * (O * O) +
-                        (oy + half_o) * O + (ox + half_o));
+    if (!drop)                       // < 2^32 (checked at plan creation); gx, gy >= 0 here
+        kk = (((uint32_t)kset * (uint32_t)nt + (uint32_t)gy / kBucketTile) * (uint32_t)nt + (uint32_t)gx / kBucketTile) * (uint32_t)(O * O) +
+             (uint32_t)((oy + half_o) * O + (ox + half_o));
     else
         atomicAdd(&counters[1], 1);
     key[k] = kk;
