@@ -179,19 +179,6 @@ __global__ void __launch_bounds__(kDedupeThreads, 2) sorted_geo_dedupe_kernel(co
     }
 }
 
-// sval[rep] += sval[i] for every merged visibility i (after gather_values_kernel)
-template <int NC>
-__global__ void accumulate_duplicates_kernel(const int32_t* __restrict__ counters, const int32_t* __restrict__ rep,
-                                             float2* __restrict__ sval) {
-    const int n_kept = counters[0];
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_kept; i += gridDim.x * blockDim.x) {
-        const int r = rep[i];
-        if (r == i) continue;
-#pragma unroll
-        for (int c = 0; c < NC; ++c) atomicAdd(&sval[(int64_t)r * NC + c], sval[(int64_t)i * NC + c]);
-    }
-}
-
 // sorted-order weighted visibilities  w_kc * V_kc
 template <int NC>
 __global__ void gather_values_kernel(const int32_t* __restrict__ counters, const int32_t* __restrict__ perm,
@@ -207,6 +194,43 @@ __global__ void gather_values_kernel(const int32_t* __restrict__ counters, const
             sval[(int64_t)i * NC + c] = make_float2(w * v.x, w * v.y);
         }
     }
+}
+
+// gather_values + accumulate_duplicates in one pass: a CTA owns one dedupe chunk (a merged visibility and its
+// representative are always in the same chunk), gathers the weighted values into shared memory, adds the merged ones
+// to their representatives there, and writes the chunk out once.
+template <int NC>
+__global__ void __launch_bounds__(1024) gather_merge_values_kernel(const int32_t* __restrict__ counters, const int32_t* __restrict__ perm,
+                                                                   const int32_t* __restrict__ rep, const float2* __restrict__ vis,
+                                                                   const float* __restrict__ weights, float2* __restrict__ sval) {
+    extern __shared__ __align__(16) unsigned char gm_smem[];
+    float2* s_val = reinterpret_cast<float2*>(gm_smem);                   // [kDedupeChunk][NC]
+    const int n_kept = counters[0];
+    const int c0 = blockIdx.x * kDedupeChunk;
+    if (c0 >= n_kept) return;
+    const int c1 = min(n_kept, c0 + kDedupeChunk);
+    for (int i = c0 + threadIdx.x; i < c1; i += blockDim.x) {
+        const int64_t k = perm[i];
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            const float2 v = vis[k * NC + c];
+            const float w = weights[k * NC + c];
+            s_val[(i - c0) * NC + c] = make_float2(w * v.x, w * v.y);
+        }
+    }
+    __syncthreads();
+    for (int i = c0 + threadIdx.x; i < c1; i += blockDim.x) {
+        const int r = rep[i];
+        if (r == i) continue;
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            const float2 v = s_val[(i - c0) * NC + c];                    // a merged one is never a representative: not modified
+            atomicAdd(&s_val[(r - c0) * NC + c].x, v.x);
+            atomicAdd(&s_val[(r - c0) * NC + c].y, v.y);
+        }
+    }
+    __syncthreads();
+    for (int q = threadIdx.x; q < (c1 - c0) * NC; q += blockDim.x) sval[(int64_t)c0 * NC + q] = s_val[q];
 }
 
 // degridding epilogue: sorted-order sums -> vis_out in input order (dropped visibilities predict 0); with `residual`
@@ -1197,6 +1221,8 @@ static int init_buffers(imager_plan* pl, TiledState* st, cudaStream_t stream) {
 #if IMAGER_DEDUPE
     IMAGER_CUDA(cudaMalloc(&st->d_rep, mv * sizeof(int32_t)));
     IMAGER_CUDA(cudaFuncSetAttribute(sorted_geo_dedupe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kDedupeSmem));
+    IMAGER_CUDA(cudaFuncSetAttribute(gather_merge_values_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     kDedupeChunk * 4 * (int)sizeof(float2)));
 #endif
     IMAGER_CUDA(cudaMalloc(&st->d_sval, mv * pl->p.n_corr * sizeof(float2)));
     IMAGER_CUDA(cudaMalloc(&st->d_total, sizeof(unsigned long long)));
@@ -1387,14 +1413,18 @@ int launch_grid_tiled(imager_plan* pl, int64_t nvis, const float2* vis, const fl
     int rc = prepare(pl, st, stream);
     if (rc) return rc;
     const unsigned gb = 4 * kNumSMs;
-    if (pl->p.n_corr == 1)
+    if (st->d_rep) {                          // duplicates pre-summed: gather and merge in one pass over the dedupe chunks
+        const unsigned chunks = (unsigned)((pl->indexed_nvis + kDedupeChunk - 1) / kDedupeChunk);
+        if (pl->p.n_corr == 1)
+            gather_merge_values_kernel<1><<<chunks, 1024, kDedupeChunk * 1 * sizeof(float2), stream>>>(
+                pl->d_counters, pl->d_perm[pl->sorted_buf], st->d_rep, vis, weights, st->d_sval);
+        else
+            gather_merge_values_kernel<4><<<chunks, 1024, kDedupeChunk * 4 * sizeof(float2), stream>>>(
+                pl->d_counters, pl->d_perm[pl->sorted_buf], st->d_rep, vis, weights, st->d_sval);
+    } else if (pl->p.n_corr == 1) {
         gather_values_kernel<1><<<gb, 256, 0, stream>>>(pl->d_counters, pl->d_perm[pl->sorted_buf], vis, weights, st->d_sval);
-    else
+    } else {
         gather_values_kernel<4><<<gb, 256, 0, stream>>>(pl->d_counters, pl->d_perm[pl->sorted_buf], vis, weights, st->d_sval);
-    if (st->d_rep) {
-        if (pl->p.n_corr == 1) accumulate_duplicates_kernel<1><<<gb, 256, 0, stream>>>(pl->d_counters, st->d_rep, st->d_sval);
-        else accumulate_duplicates_kernel<4><<<gb, 256, 0, stream>>>(pl->d_counters, st->d_rep, st->d_sval);
-        pl->last_launches += 1;
     }
     IMAGER_CUDA(cudaMemsetAsync(pl->d_counters + 8, 0, sizeof(int32_t), stream));
     TiledArgs a;
