@@ -64,7 +64,7 @@ constexpr int kGridThreads = IMAGER_GRID_THREADS;     // gridding kernel: thread
 #endif
 constexpr int kItemHits = IMAGER_ITEM_HITS;                        // hits per work item (one flush / strip load each)
 constexpr int kBlockHits = IMAGER_BLOCK_HITS;                     // hits per CTA-level block
-constexpr int kStageBytes = kWarps * 32 * 16;         // per-warp hit descriptors (degridding)
+constexpr int kStageBytes = kWarps * 32 * 8;          // per-warp hit descriptors (degridding): 32 x {tap address, sorted index}
 constexpr int kStageSlots = 40;                       // gridding: 32 descriptors + the one read past a batch's end
 constexpr int kGridStageBytes = (kGridThreads / 32) * kStageSlots * 16;
 constexpr int kMaxSmem = 227 * 1024;
@@ -74,6 +74,7 @@ constexpr int kMaxSmem = 227 * 1024;
 constexpr int kRedSlots = IMAGER_RED_SLOTS;            // degridding: hits per transposed reduction (8, 16 or 32)
 constexpr int kRedBytes = kWarps * kRedSlots * 32 * 8;
 constexpr int kTableBudget = kMaxSmem - (kStageBytes + kRedBytes > kGridStageBytes ? kStageBytes + kRedBytes : kGridStageBytes) - 1024;   // 1 KB: static
+static_assert(kTableBudget >= (127 + 2 * kPadY) * 152 * 8, "a support-127 slice (BASELINE.json configs[4]: 133 rows x 152 taps) must fit the table budget");
 constexpr int64_t kMaxPlanCells = (int64_t)1 << 30;   // (geometry unit, strip) pairs: 12 bytes of planner state each
 constexpr uint32_t kTapBias = 1u << 20;
 

@@ -66,6 +66,7 @@ def test_config5_chunked_grid_fft_degrid_round_trip(oracle_lib):
             wts = torch.from_numpy(wl.weights).cuda()
             plan.grid(uvw, vis, wts, grid, a, sumwt, flags=1)        # accumulates: the index is the one just built
             torch.cuda.synchronize()
+            assert plan.index_stats()["n_hits"] > 0, "support 127 must run on the tiled path (its slice has to fit the table budget)"
             del vis, wts, uvw, a
             if cells is None:                                       # half at visibility positions, half across the coverage
                 pick = rng.integers(0, wl.nvis, 1500)
