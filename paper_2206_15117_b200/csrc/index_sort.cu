@@ -22,12 +22,11 @@ __device__ __forceinline__ int floor_div32(int a, int b) {      // b > 0
     return (a - q * b < 0) ? q - 1 : q;
 }
 
-__global__ void index_kernel(int64_t nvis, const float* __restrict__ uvw, const int32_t* __restrict__ a_index,
-                             double uv_scale, double w_scale, int N, int O, int P, int nt, int n_aplanes, uint32_t key_drop,
-                             const int32_t* __restrict__ plane_support, imager_record* __restrict__ rec,
-                             uint32_t* __restrict__ key, int32_t* __restrict__ counters) {   // the permutation starts as the identity: first sort pass
-    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= nvis) return;
+// record and sort key of visibility k (the permutation starts as the identity: the first sort pass assumes it)
+__device__ __forceinline__ uint32_t index_one(int64_t k, const float* __restrict__ uvw, const int32_t* __restrict__ a_index,
+                                              double uv_scale, double w_scale, int N, int O, int P, int nt, int n_aplanes,
+                                              uint32_t key_drop, const int32_t* __restrict__ plane_support,
+                                              imager_record* __restrict__ rec, int32_t* __restrict__ counters) {
     float u = uvw[3 * k], v = uvw[3 * k + 1], w = uvw[3 * k + 2];
     int a = a_index ? a_index[k] : 0;
     const double su = __dmul_rn((double)u, uv_scale), sv = __dmul_rn((double)v, uv_scale);
@@ -41,8 +40,7 @@ __global__ void index_kernel(int64_t nvis, const float* __restrict__ uvw, const 
         r.kset = 0;
         rec[k] = r;
         atomicAdd(&counters[1], 1);
-        key[k] = key_drop;
-        return;
+        return key_drop;
     }
     // |su|, |sv| < 2^30 from here on: 32-bit integer arithmetic gives the same values as the 64-bit definition
     const int qx = __double2int_rn(su), qy = __double2int_rn(sv);
@@ -69,8 +67,37 @@ __global__ void index_kernel(int64_t nvis, const float* __restrict__ uvw, const 
              (uint32_t)((oy + half_o) * O + (ox + half_o));
     else
         atomicAdd(&counters[1], 1);
-    key[k] = kk;
+    return kk;
 }
+
+// One CTA indexes one sort tile (kSortChunk visibilities) and leaves the tile's histogram of the first radix digit, so
+// that the first sort pass needs no histogram pass of its own.  hist[d * n_tiles + tile], as radix_hist_kernel writes it.
+__global__ void __launch_bounds__(256) index_kernel(int64_t nvis, const float* __restrict__ uvw, const int32_t* __restrict__ a_index,
+                                                    double uv_scale, double w_scale, int N, int O, int P, int nt, int n_aplanes,
+                                                    uint32_t key_drop, const int32_t* __restrict__ plane_support,
+                                                    imager_record* __restrict__ rec, uint32_t* __restrict__ key,
+                                                    int32_t* __restrict__ counters, int32_t* __restrict__ hist, int n_tiles) {
+    __shared__ int32_t cnt[8][256];
+    const int warp = threadIdx.x >> 5;
+    for (int i = threadIdx.x & 31; i < 256; i += 32) cnt[warp][i] = 0;
+    __syncwarp();
+    const int64_t base = (int64_t)blockIdx.x * kSortChunk;
+#pragma unroll 2
+    for (int r = 0; r < kSortChunk / 256; ++r) {
+        const int64_t k = base + r * 256 + threadIdx.x;
+        if (k < nvis) {
+            const uint32_t kk = index_one(k, uvw, a_index, uv_scale, w_scale, N, O, P, nt, n_aplanes, key_drop, plane_support, rec, counters);
+            key[k] = kk;
+            atomicAdd(&cnt[warp][kk & 255u], 1);
+        }
+    }
+    __syncthreads();
+    int t = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) t += cnt[w][threadIdx.x];
+    hist[(int64_t)threadIdx.x * n_tiles + blockIdx.x] = t;
+}
+
 
 // ---- radix sort: one CTA owns a tile of kSortChunk consecutive items (8 warps x kSortRows rows of 32) ----
 constexpr int kSortThreads = 256, kSortWarps = kSortThreads / 32, kSortRows = kSortChunk / kSortThreads;
@@ -235,11 +262,42 @@ __global__ void scan_add_kernel(int32_t* __restrict__ data, const int32_t* __res
     }
 }
 
+// data[i] += sum of the block totals before block i / 1024: every block sums its predecessors' totals itself (at most
+// kDirectBlocks of them), which saves the scan of the totals and one launch per level
+constexpr int kDirectBlocks = 4096;
+__global__ void scan_add_direct_kernel(int32_t* __restrict__ data, const int32_t* __restrict__ block_sums, int64_t n) {
+    __shared__ int32_t warp_tot[8];
+    __shared__ int32_t s_off;
+    int32_t t = 0;
+    for (int j = threadIdx.x; j < (int)blockIdx.x; j += 256) t += block_sums[j];
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) t += __shfl_xor_sync(0xffffffffu, t, d);
+    if ((threadIdx.x & 31) == 0) warp_tot[threadIdx.x >> 5] = t;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int32_t o = 0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) o += warp_tot[w];
+        s_off = o;
+    }
+    __syncthreads();
+    const int32_t off = s_off;
+    const int64_t i = (int64_t)blockIdx.x * 1024 + threadIdx.x;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const int64_t idx = i + j * 256;
+        if (idx < n) data[idx] += off;
+    }
+}
+
 static int exclusive_scan(imager_plan* pl, int32_t* data, int64_t n, int32_t* tmp, cudaStream_t st) {
     const int64_t nb = (n + 1023) / 1024;
     scan_block_kernel<<<(unsigned)nb, 256, 0, st>>>(data, data, nb > 1 ? tmp : nullptr, n);
     pl->last_launches++;
-    if (nb > 1) {
+    if (nb > 1 && nb <= kDirectBlocks) {
+        scan_add_direct_kernel<<<(unsigned)nb, 256, 0, st>>>(data, tmp, n);
+        pl->last_launches++;
+    } else if (nb > 1) {
         int rc = exclusive_scan(pl, tmp, nb, tmp + nb, st);
         if (rc) return rc;
         scan_add_kernel<<<(unsigned)nb, 256, 0, st>>>(data, tmp, n);
@@ -271,9 +329,10 @@ int run_index_and_sort(imager_plan* pl, int64_t nvis, const float* uvw, const in
     const imager_params& p = pl->p;
     IMAGER_CUDA(cudaMemsetAsync(pl->d_counters, 0, 64 * sizeof(int32_t), st));
     if (nvis > 0) {
-        index_kernel<<<(unsigned)((nvis + 255) / 256), 256, 0, st>>>(
+        index_kernel<<<(unsigned)((nvis + kSortChunk - 1) / kSortChunk), 256, 0, st>>>(
             nvis, uvw, a_index, pl->uv_scale, pl->w_scale, p.grid_size, p.oversample, p.n_wplanes, pl->nt, p.n_aplanes,
-            pl->key_drop, pl->d_plane_support, pl->d_rec, pl->d_key[0], pl->d_counters);
+            pl->key_drop, pl->d_plane_support, pl->d_rec, pl->d_key[0], pl->d_counters, pl->d_hist,
+            (int)((nvis + kSortChunk - 1) / kSortChunk));
         pl->last_launches++;
     }
     int cur = 0;
@@ -281,8 +340,10 @@ int run_index_and_sort(imager_plan* pl, int64_t nvis, const float* uvw, const in
     for (int pass = 0; pass < pl->sort_passes && nvis > 0; ++pass) {
         const int shift = 8 * pass;
         const unsigned blocks = (unsigned)n_chunks;
-        radix_hist_kernel<<<blocks, kSortThreads, 0, st>>>(nvis, pl->d_key[cur], shift, pl->d_hist, n_chunks);
-        pl->last_launches++;
+        if (pass > 0) {                           // the index kernel has left the histograms of the first digit
+            radix_hist_kernel<<<blocks, kSortThreads, 0, st>>>(nvis, pl->d_key[cur], shift, pl->d_hist, n_chunks);
+            pl->last_launches++;
+        }
         int rc = exclusive_scan(pl, pl->d_hist, (int64_t)256 * n_chunks, pl->d_scan_tmp, st);
         if (rc) return rc;
         radix_scatter_kernel<<<blocks, kSortThreads, 0, st>>>(nvis, pl->d_key[cur], pass == 0 ? nullptr : pl->d_perm[cur],
