@@ -126,7 +126,7 @@ __global__ void __launch_bounds__(kSortThreads) radix_hist_kernel(int64_t n, con
 // __match_any_sync (rank = lower peers), per-warp digit counters order the rows, a prefix over the warps orders the
 // warps: the tile is first sorted by digit in shared memory, then written out in runs of equal digit (coalesced), each
 // run to the place the scanned histograms give it.  val_in == nullptr: the values are the input indices (first pass).
-__global__ void __launch_bounds__(kSortThreads) radix_scatter_kernel(int64_t n, const uint32_t* __restrict__ key_in,
+__global__ void __launch_bounds__(kSortThreads, 3) radix_scatter_kernel(int64_t n, const uint32_t* __restrict__ key_in,
                                                                      const int32_t* __restrict__ val_in,
                                                                      uint32_t* __restrict__ key_out, int32_t* __restrict__ val_out,
                                                                      int shift, const int32_t* __restrict__ hist_scanned, int n_tiles) {
