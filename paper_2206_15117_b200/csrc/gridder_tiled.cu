@@ -18,10 +18,11 @@
 //       LDS.128 (value and tap address, loaded a hit ahead) and straight-line code specialised for the range
 //       (1 LDS.64 + 2 FFMA2 per slot, nothing else);
 //   (4) gridding flushes a strip once per work item with red.global.add.v2.f32; degridding loads the strip once
-//       per item, writes each hit's 32 partial sums with one STS.64, sums 8 hits at a time by a transposed read and
-//       two shuffles, and adds the result to the visibility with one red.global.add.v2.f32.
-// Work planning (visibility-centric, warp-aggregated atomics): hits per (geometry unit, strip) are counted, scanned,
-// emitted and counting-sorted by slot-range variant; item = up to kItemHits hits of one (unit, strip); block =
+//       per item, writes each hit's 32 partial sums with one STS.64, sums 16 hits at a time by a transposed read and
+//       one shuffle stage, and adds the result to the visibility with one red.global.add.v2.f32.
+// Work planning (visibility-centric; a warp counts the lanes that meet each strip of its window with one ballot and
+// issues one atomic per strip): hits per (geometry unit, strip) are counted, scanned, emitted and counting-sorted by
+// slot-range variant; item = up to kItemHits hits of one (unit, strip); block =
 // consecutive items of one unit with about kBlockHits hits, times one Mueller element (s, c); persistent CTAs pull
 // blocks from a two-ended global queue (small blocks last), their warps pull items of the block from a shared counter.
 #include "common.cuh"
@@ -910,8 +911,8 @@ grid_tiled_kernel(const TiledArgs a, const float2* __restrict__ sval, float2* __
 // ---- degridding ------------------------------------------------------------------------------------------
 // Same hits, same ownership: the warp holds its strip of the grid in registers; a hit's lanes accumulate
 // sum conj(t) g over their cells:  P += t * g.x, Q += t * g.y,  conj(t) g = (P.x + Q.y) + i (Q.x - P.y).
-// The 32 partial sums of a hit go to a per-warp shared buffer red[slot][lane]; every 8 hits the buffer is summed
-// by a transposed read (lane = slot + 8 * quarter sums 8 columns, two shuffles join the quarters) and the result is
+// The 32 partial sums of a hit go to a per-warp shared buffer red[slot][lane]; every kRedSlots = 16 hits the buffer is
+// summed by a transposed read (lane = slot + 16 * half sums 16 columns, one shuffle stage joins the halves) and the result is
 // added to the visibility's sorted-order sum with one red.global.add.v2.f32 per hit.  (Measured alternative, DESIGN.md
 // section 6.4: the same sum by one mma.sync.m16n8k8 per hit with a TF32 head / tail split takes the reduction off the
 // shared-memory pipe -- 77 % -> 54 % busy -- but the longer bodies miss the instruction cache more: 4.9 ms against 4.1.)
@@ -1049,7 +1050,7 @@ degrid_tiled_kernel(const TiledArgs a, const float2* __restrict__ grid, float2* 
 #undef IMAGER_BODY_ARGS
                     h += cnt;
                     if ((h & (kRedSlots - 1)) == 0 || h == n) {
-                        // transposed reduction of hits [h0, h): lane = slot + 8 * quarter sums columns 8 q .. 8 q + 7
+                        // transposed reduction of hits [h0, h)
                         const int h0 = (h - 1) & ~(kRedSlots - 1);
                         __syncwarp();
                         // lane = slot + kRedSlots * part sums the kRedCols columns of its part
