@@ -1,9 +1,10 @@
 """Oracle for the minor cycle and the Cotton-Schwab loop.  TEST INFRASTRUCTURE (oracle/__init__.py).
 
-Paper: "These images are then cleaned using the Cotton-Schwab algorithm ... Input parameters include ... the number of
-clean cycles, loop gain, cycle factor, threshold"; the Hogbom minor cycle is named among the stages suited
-to the GPU.  The paper gives neither algorithm in symbols; what follows is the textbook statement
-(readings R18-R20):
+Paper: "The output images are cleaned using an implementation of the Cotton-Schwab algorithm [6], which accepts many of
+the usual parameters such as the number of clean cycles, the loop gain, the cycle factor, and a threshold stopping
+criterion".  Of the minor cycle the paper says only that "more iterative processes such as Högbom cleaning
+[10] are less able to take full advantage of parallelisation".  The paper gives neither algorithm in
+symbols; what follows is the textbook statement (readings R18-R20):
 
   Hogbom minor cycle (R18) on a real residual image R, a PSF B with B[c, c] = 1 at c = N/2, inside a window W:
       repeat up to n_iter times:

@@ -1,7 +1,9 @@
 // clean.cu -- the minor cycle and the Cotton-Schwab major-cycle loop around the hot path.
 //
-// PAPER.md:27 "These images are then cleaned using the Cotton-Schwab algorithm ... the number of clean cycles, loop gain,
-// cycle factor, threshold"; PAPER.md:110 names the Hogbom minor cycle among the stages that suit the GPU.  The paper gives
+// PAPER.md:27 "The output images are cleaned using an implementation of the Cotton-Schwab algorithm [6], which accepts many
+// of the usual parameters such as the number of clean cycles, the loop gain, the cycle factor, and a threshold stopping
+// criterion"; PAPER.md:110 counts Hogbom cleaning among the "more iterative processes" that "are less able to take full
+// advantage of parallelisation" (hence the device-side control below: the host never waits on it).  The paper gives
 // neither in symbols; readings R18-R20 state them:
 //   R18  Hogbom: p = first pixel (row-major) of the window with the largest |R|; a = gain * R[p]; model[p] += a;
 //        R[q] -= a * B[q - p + c] wherever that PSF sample exists (c = N/2); up to n_iter times.

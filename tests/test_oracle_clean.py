@@ -103,3 +103,36 @@ def test_cotton_schwab_recovers_three_point_sources(oracle_lib):
         assert abs(out["model"][n // 2 + py, n // 2 + px] - a) < 0.1 * a + 0.02
     assert np.abs(out["residual_vis"]).mean() < 0.1 * np.abs(vis).mean()
     assert len(out["cycles"]) == 5 and len(out["cycles"][0]) > 3
+
+
+def test_float64_pixel_loop_finds_the_same_peaks():
+    """The oracle works in float32 on purpose (the peak search decides an integer; header of oracle/clean.py).  Pin its
+    decisions against R18 written out once more in float64 with plain pixel loops: while successive peaks are separated
+    by far more than float32 rounding, both must find the same pixels in the same order, and values within 1e-5."""
+    n, c = 24, 12
+    psf = _gauss_psf(n, width=1.5, sidelobe=0.15)
+    r32 = np.zeros((n, n), np.float32)
+    for py, px, a in [(7, 15, 3.0), (16, 6, -2.2), (11, 11, 1.3)]:
+        for y in range(n):
+            for x in range(n):
+                if 0 <= y - py + c < n and 0 <= x - px + c < n:
+                    r32[y, x] += np.float32(a) * psf[y - py + c, x - px + c]
+    gain, n_iter = 0.35, 12
+    out = oc.hogbom(r32, psf, (2, 2, 22, 22), gain=gain, threshold=0.0, cycle_factor=0.0, n_iter=n_iter)
+    r, b, found = r32.astype(np.float64), psf.astype(np.float64), []
+    for _ in range(n_iter):
+        best, p = -1.0, None
+        for y in range(2, 22):
+            for x in range(2, 22):
+                if abs(r[y, x]) > best:                                  # strict: the first maximum in row-major order
+                    best, p = abs(r[y, x]), (y, x)
+        a = gain * r[p]
+        found.append((p[0], p[1], a))
+        for y in range(n):
+            for x in range(n):
+                if 0 <= y - p[0] + c < n and 0 <= x - p[1] + c < n:
+                    r[y, x] -= a * b[y - p[0] + c, x - p[1] + c]
+    assert [k[:2] for k in out["components"]] == [k[:2] for k in found]
+    assert len({k[:2] for k in found}) >= 3
+    assert np.allclose([k[2] for k in out["components"]], [k[2] for k in found], rtol=0, atol=1e-5)
+    assert np.abs(out["residual"] - r).max() < 1e-5

@@ -131,6 +131,50 @@ def test_eq1_single_pointing_and_airy():
     assert abs(ok.airy(first_null, 12.0, 1e9)) < 1e-6
 
 
+def test_eq1_several_pointings_by_hand():
+    """Eq. 1 with N > 1, where sum B_i^2, (sum B_i)^2 and the max term can be told apart.  Values worked by
+    hand from the printed formula gamma = [sqrt(sum B_i^2) / max sqrt(sum B_i^2)] [1 / sum B_i^2]."""
+    # two flat beams B_1 = 1, B_2 = b: sum B^2 = 1 + b^2 everywhere, the first bracket is 1, gamma = 1 / (1 + b^2)
+    # ((sum B)^2 would give 1 / (1 + b)^2 = 0.4444, a plain mean 1 / ((1 + b^2) / 2) = 1.6)
+    b = 0.5
+    g = oi.mosaic_gamma(np.array([np.ones((3, 4)), np.full((3, 4), b)]))
+    assert g.shape == (3, 4) and np.allclose(g, 0.8, rtol=0, atol=1e-15)
+    # two pixels, two beams: B_1 = (1, 1/2), B_2 = (1/2, 1/5)  =>  sum B^2 = (5/4, 29/100); the maximum of the root is at
+    # pixel 0, so gamma_0 = 1 / (5/4) = 0.8 and gamma_1 = sqrt(29/100) / sqrt(5/4) / (29/100) = sqrt(0.232) / 0.29
+    g = oi.mosaic_gamma(np.array([[1.0, 0.5], [0.5, 0.2]]))
+    assert abs(g[0] - 0.8) < 1e-15
+    assert abs(g[1] - 1.6609095970747993) < 1e-14                  # 0.48166378315169184 / 0.29, by hand calculator
+    # three beams that never overlap: each pixel sees one beam, gamma = 1 / (B max B) as for a single pointing
+    beams = np.array([[0.9, 0.0, 0.0], [0.0, 0.6, 0.0], [0.0, 0.0, 0.3]])
+    assert np.allclose(oi.mosaic_gamma(beams), 1.0 / (np.array([0.9, 0.6, 0.3]) * 0.9), rtol=1e-15)
+
+
+def test_R10_rotation_sense_and_eq5_on_a_rotation():
+    """Reading R10 (J = E D R(chi)) and Eq. 5 pinned on what the mathematics fixes: a rotation of the feeds
+    by chi, R = [[cos, -sin], [sin, cos]] acting on (E_x, E_y), leaves Stokes I and V alone and turns (Q, U) by +2 chi:
+    a field along x (XX = 1: I = Q = 1/2, U = 0) becomes (cos chi, sin chi), i.e. XX = cos^2, YY = sin^2, XY = YX =
+    sin cos, so Q = cos(2 chi)/2 and U = +sin(2 chi)/2.  A transposed rotation flips the sign of the U term; S and S^-1
+    swapped in Eq. 5 does not give a real rotation at all."""
+    chi = 0.3
+    j = ok.jones_matrix([0.0, 0.0], chi)
+    assert np.allclose(j @ np.array([1.0, 0.0]), [np.cos(chi), np.sin(chi)], atol=1e-15)
+    ms = ok.mueller_stokes(ok.mueller(j, j))
+    c2, s2 = 0.8253356149096783, 0.5646424733950354                # cos 0.6, sin 0.6
+    want = np.array([[1, 0, 0, 0], [0, c2, -s2, 0], [0, s2, c2, 0], [0, 0, 0, 1]], dtype=np.complex128)
+    assert np.allclose(ms, want, atol=1e-15)
+    assert np.allclose(ms @ [0.5, 0.5, 0, 0], [0.5, 0.5 * c2, +0.5 * s2, 0], atol=1e-15)     # the worked example above
+    # Eq. 5 on a matrix that is not a rotation: pure gain difference g_x = 1, g_y = k mixes I and Q only, as
+    # I' = (1 + k^2)/2 I + (1 - k^2)/2 Q and Q' = (1 - k^2)/2 I + (1 + k^2)/2 Q, and scales U and V by k
+    k = 0.8
+    jg = np.diag([1.0, k])
+    mg = ok.mueller_stokes(ok.mueller(jg, jg))
+    p, m = (1 + k * k) / 2, (1 - k * k) / 2
+    assert np.allclose(mg, [[p, m, 0, 0], [m, p, 0, 0], [0, 0, k, 0], [0, 0, 0, k]], atol=1e-15)
+    # leakage enters on the left of the rotation (D R), so at chi = pi/2 it is the SECOND column of D that meets E_x
+    jl = ok.jones_matrix([0.01, 0.02j], np.pi / 2)
+    assert np.allclose(jl @ np.array([1.0, 0.0]), [0.01, 1.0], atol=1e-15)
+
+
 def test_awproj_tables_structure():
     """ADJOINT tables are (M S^-1)^H element by element times the scalar w-kernel; PAPER-mode gridding tables
     invert the regularised Stokes Mueller matrix: with zero leakage and a flat beam they reduce to S itself."""
