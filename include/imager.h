@@ -169,6 +169,34 @@ int imager_hogbom(float* residual, const float* psf, float* model, int32_t n, co
                   float threshold, float cycle_factor, int32_t n_iter, float* components_out, int32_t* n_components_out,
                   void* cuda_stream);
 
+/* The same minor cycle for callers that must not allocate device memory.  imager_hogbom above takes three small scratch
+ * buffers from the stream-ordered pool (cudaMallocAsync / cudaFreeAsync) on every call.  Some users of this library cannot
+ * do that: a pipeline that shares one GPU with a correlator or beamformer and had all of its HBM handed out at start-up, a
+ * process in which a framework's caching allocator already owns the device, a real-time loop that cannot take the
+ * allocator's locks, pool growth or the device-wide wait that cudaMalloc / cudaFree can cause.  This entry point calls no
+ * cudaMalloc, cudaMallocAsync, cudaFree or any library routine that allocates; its scratch is an array built into
+ * libimager.so (file-scope `static __device__` in csrc/clean.cu): 131,328 bytes (256 of control block + 16384 per-block peak
+ * records of 8 bytes), held by EVERY GPU that loads the library from the moment it is loaded until the process exits,
+ * used or not.  The caller still passes every input and output.
+ *   - Arguments, arithmetic, results and stream behaviour are those of imager_hogbom: residual / model / components are
+ *     bit-identical between the two calls.  Enqueues 2 n_iter + 5 kernels, never synchronises.
+ *   - Limit: n <= IMAGER_HOGBOM_STATIC_MAX_N (the scratch holds one peak record per 1024 pixels of a 4096 x 4096 image).
+ *     A larger n is refused with IMAGER_ERR_UNSUPPORTED and a message naming the limit; nothing is enqueued.
+ *   - Set-up: the FIRST call on each device (with that device current) looks up the array's device address
+ *     (cudaGetSymbolAddress, return code checked; the first use may also make the CUDA runtime load the library's module
+ *     on that device) and keeps it for later calls on that device.  Make that first call ahead of time: before any stream
+ *     capture is begun, and outside whatever section of the caller's loop may not make such runtime calls.
+ *   - One array per GPU, shared by every call in the process.  It keeps the previous call's contents; the entry point
+ *     rewrites what has to start from zero (the control block) at the head of its own work queue, so back-to-back calls on
+ *     ONE stream are fine.  Two calls whose kernels can overlap on the same GPU (different streams without an ordering
+ *     event, different host threads) RACE on the array and give wrong results: order them, or use imager_hogbom for all
+ *     but one of them.
+ * Errors: INVALID_ARG (NULL, n < 2), UNSUPPORTED (n beyond the limit; device ordinal >= 64), CUDA. */
+#define IMAGER_HOGBOM_STATIC_MAX_N 4096
+int imager_hogbom_static(float* residual, const float* psf, float* model, int32_t n, const int32_t window[4], float gain,
+                         float threshold, float cycle_factor, int32_t n_iter, float* components_out,
+                         int32_t* n_components_out, void* cuda_stream);
+
 typedef struct imager_clean_params {
     int32_t n_major;          /* major (Cotton-Schwab) cycles, >= 1 ("number of clean cycles")                      */
     int32_t n_iter;           /* minor-cycle iterations per major cycle                                                    */

@@ -3,7 +3,7 @@
 The product is `libimager.so` (CUDA, sm_100a; C-ABI in include/imager.h).  This package is its thin Python
 binding: the four hot-path calls keep their C names.  Nothing here computes anything on the CPU.
 """
-from .binding import (ImagerError, Plan, load_library, hogbom as imager_hogbom, reproject as imager_reproject, MODE_DELTA, MODE_PSWF, MODE_WPROJ, MODE_AWPROJ_ADJOINT,
+from .binding import (ImagerError, Plan, load_library, hogbom as imager_hogbom, hogbom_static as imager_hogbom_static, reproject as imager_reproject, MODE_DELTA, MODE_PSWF, MODE_WPROJ, MODE_AWPROJ_ADJOINT,
                       MODE_AWPROJ_PAPER, MODE_MOSAIC_PB, MODE_USER, REUSE_INDEX, PATH_REFERENCE, DEGRID_RESIDUAL, EXPORTS)
 
 

@@ -22,7 +22,7 @@ DEGRID_RESIDUAL = 16
 
 EXPORTS = ("imager_plan_create", "imager_index", "imager_grid", "imager_degrid", "imager_plan_destroy",
            "imager_grid_image_transform", "imager_mosaic_correct", "imager_debug_index", "imager_debug_kernels", "imager_plan_info",
-           "imager_index_stats", "imager_hogbom", "imager_clean", "imager_reproject", "imager_mosaic_grid",
+           "imager_index_stats", "imager_hogbom", "imager_hogbom_static", "imager_clean", "imager_reproject", "imager_mosaic_grid",
            "imager_mosaic_degrid",
            "imager_last_launch_count", "imager_debug_violations", "imager_last_error")
 
@@ -77,6 +77,7 @@ def load_library() -> ctypes.CDLL:
                                          c_int32, c_double, POINTER(c_void_p), c_uint32, c_void_p]
     lib.imager_hogbom.argtypes = [c_void_p, c_void_p, c_void_p, c_int32, POINTER(c_int32), c_float, c_float, c_float, c_int32,
                                   c_void_p, c_void_p, c_void_p]
+    lib.imager_hogbom_static.argtypes = lib.imager_hogbom.argtypes
     lib.imager_clean.argtypes = [c_void_p, c_int64, c_void_p, c_void_p, c_void_p, c_void_p, POINTER(ImagerCleanParams), c_void_p,
                                  c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
     lib.imager_last_launch_count.argtypes = [c_void_p]
@@ -295,6 +296,26 @@ def hogbom(residual, psf, model, window, gain: float, threshold: float, cycle_fa
         _dev_ptr(residual, torch.float32, "residual"), _dev_ptr(psf, torch.float32, "psf"), _dev_ptr(model, torch.float32, "model"),
         n, win, float(gain), float(threshold), float(cycle_factor), int(n_iter), _dev_ptr(components_out, torch.float32, "components_out"),
         _dev_ptr(n_components_out, torch.int32, "n_components_out"), _stream_ptr(stream)), "imager_hogbom")
+
+
+HOGBOM_STATIC_MAX_N = 4096
+
+
+def hogbom_static(residual, psf, model, window, gain: float, threshold: float, cycle_factor: float, n_iter: int,
+                  components_out=None, n_components_out=None, stream=None):
+    """imager_hogbom_static: the minor cycle of `hogbom`, same arguments and bit-identical results, for callers that may not
+    allocate device memory (all HBM handed out at start-up, a caching allocator that owns the device, a real-time loop).
+    The library calls no allocator here: its scratch is a 128 KB array built into libimager.so and shared by every call on
+    that GPU, so images are limited to HOGBOM_STATIC_MAX_N pixels a side (ImagerError otherwise) and two calls that can
+    overlap on one GPU race.  The first call on a device also looks up the array's address: make it before any stream
+    capture.  (This Python wrapper itself allocates nothing on the device; the tensors are the caller's.)"""
+    import torch
+    n = int(residual.shape[-1])
+    win = (c_int32 * 4)(*[int(v) for v in window])
+    _check(load_library().imager_hogbom_static(
+        _dev_ptr(residual, torch.float32, "residual"), _dev_ptr(psf, torch.float32, "psf"), _dev_ptr(model, torch.float32, "model"),
+        n, win, float(gain), float(threshold), float(cycle_factor), int(n_iter), _dev_ptr(components_out, torch.float32, "components_out"),
+        _dev_ptr(n_components_out, torch.int32, "n_components_out"), _stream_ptr(stream)), "imager_hogbom_static")
 
 
 def reproject(src, cell_src: float, dst, cell_dst: float, shift_lm, beam: int = 0, dish_diameter_m: float = 0.0,

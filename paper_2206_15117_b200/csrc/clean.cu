@@ -20,6 +20,7 @@
 // `hogbom_pick_kernel` (one block: the global peak, the stop test, the new component).  The host never reads anything
 // back: once the stop test fails the remaining launches see `done` and return at once.
 #include "common.cuh"
+#include <mutex>
 
 namespace imager {
 
@@ -285,4 +286,111 @@ extern "C" int imager_clean(imager_plan* plan, int64_t nvis, const float* uvw, c
 #undef CLEAN_CUDA
 #undef CLEAN_RC
     return done(0);
+}
+
+// ---- the minor cycle for callers that may not allocate (imager_hogbom_static) ------------------------------------------
+//
+// imager_hogbom takes its three scratch buffers (control block, per-block peak values, per-block peak indices) from the
+// stream-ordered pool on every call.  That is no good to a caller whose device memory was shared out once at start-up and
+// who must not touch the allocator afterwards: an imaging loop that sits beside a correlator or beamformer on the same GPU
+// with every byte of HBM already promised, a process running under a framework whose caching allocator owns the whole
+// device, or a real-time loop that cannot afford the allocator's locks, its possible pool growth or the device-wide wait a
+// cudaMalloc / cudaFree may bring.  For them the same kernels run here on scratch that is part of the library image: a
+// file-scope device array, resident on every GPU that loads libimager.so from the moment the module is loaded until the
+// process exits, whether or not this entry point is ever called.
+//
+// Size: 256 bytes of control block + one (value, index) pair per thread block, one block per 1024 pixels, sized for
+// images up to IMAGER_HOGBOM_STATIC_MAX_N = 4096 pixels a side: 256 + 16384 * 8 = 131,328 bytes per GPU.
+//
+// `g_hogbom_scratch` below is a DEVICE symbol.  Device code may name it; in host code the identifier is only the host
+// shadow of the symbol and is NOT a device address (handing `g_hogbom_scratch` itself to a kernel would fault, or on a
+// system where the GPU can reach host memory quietly work on the wrong bytes).  Host code gets the real address once per
+// device from cudaGetSymbolAddress, with that device current, and passes that pointer to the kernels.
+namespace imager {
+
+constexpr int kStaticMaxN = IMAGER_HOGBOM_STATIC_MAX_N;
+constexpr int kStaticPixelsPerBlock = 1024;                                            // 256 threads x 4 pixels
+constexpr int kStaticMaxParts = (kStaticMaxN / 32) * (kStaticMaxN / 32);               // 16384 blocks at the largest image
+constexpr size_t kStaticCtrlBytes = 256;
+constexpr size_t kStaticScratchBytes = kStaticCtrlBytes + (size_t)kStaticMaxParts * (sizeof(float) + sizeof(int32_t));
+constexpr int kStaticMaxDevices = 64;
+static_assert(sizeof(HogbomCtrl) <= kStaticCtrlBytes, "control block outgrew its slot");
+static_assert((int64_t)kStaticMaxParts * kStaticPixelsPerBlock == (int64_t)kStaticMaxN * kStaticMaxN, "block count of the largest image");
+
+static __device__ __align__(256) unsigned char g_hogbom_scratch[kStaticScratchBytes];
+
+static std::mutex g_static_mutex;
+static unsigned char* g_static_addr[kStaticMaxDevices] = {};       // device address of g_hogbom_scratch, per device ordinal
+
+// The array keeps whatever the previous call left in it: the control block is rewritten in full here (the sidelobe level
+// is built with atomicMax and the counters are incremented, so both must start from zero); the per-block pairs need no
+// clearing, every block of an update launch overwrites its own pair before the pick kernel reads it.
+__global__ void hogbom_static_reset_kernel(HogbomCtrl* __restrict__ ctrl, int done) {
+    HogbomCtrl c;
+    c.a = 0.f;
+    c.p = -1;
+    c.stop = 0.f;
+    c.done = done;
+    c.n_comp = 0;
+    c.iter = 0;
+    c.sidelobe = 0.f;
+    c.pad = 0;
+    *ctrl = c;
+}
+
+// Set-up, once per device: resolve the device address of the scratch array for the CURRENT device and remember it.
+static int static_scratch_address(unsigned char** out) {
+    int dev = -1;
+    IMAGER_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) {
+        set_error("imager_hogbom_static: device ordinal %d is outside the %d this build keeps addresses for", dev, kStaticMaxDevices);
+        return IMAGER_ERR_UNSUPPORTED;
+    }
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[dev]) {
+        void* p = nullptr;
+        IMAGER_CUDA(cudaGetSymbolAddress(&p, g_hogbom_scratch));
+        if (!p) {
+            set_error("imager_hogbom_static: cudaGetSymbolAddress returned a null address");
+            return IMAGER_ERR_CUDA;
+        }
+        g_static_addr[dev] = static_cast<unsigned char*>(p);
+    }
+    *out = g_static_addr[dev];
+    return 0;
+}
+
+}  // namespace imager
+
+extern "C" int imager_hogbom_static(float* residual, const float* psf, float* model, int32_t n, const int32_t window[4],
+                                    float gain, float threshold, float cycle_factor, int32_t n_iter, float* components_out,
+                                    int32_t* n_components_out, void* cuda_stream) {
+    if (!residual || !psf || !model || !window || n < 2) {
+        set_error("imager_hogbom_static: NULL argument or bad size");
+        return IMAGER_ERR_INVALID_ARG;
+    }
+    if (n > kStaticMaxN) {
+        set_error("imager_hogbom_static: image side n = %d exceeds IMAGER_HOGBOM_STATIC_MAX_N = %d (the built-in scratch holds one "
+                  "peak per 1024 pixels of a %d x %d image); use imager_hogbom, which allocates, for larger images",
+                  n, kStaticMaxN, kStaticMaxN, kStaticMaxN);
+        return IMAGER_ERR_UNSUPPORTED;
+    }
+    unsigned char* base = nullptr;
+    if (int rc = static_scratch_address(&base)) return rc;
+    HogbomCtrl* ctrl = reinterpret_cast<HogbomCtrl*>(base);
+    float* part_val = reinterpret_cast<float*>(base + kStaticCtrlBytes);
+    int32_t* part_idx = reinterpret_cast<int32_t*>(base + kStaticCtrlBytes + (size_t)kStaticMaxParts * sizeof(float));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int y0 = std::max(0, window[0]), x0 = std::max(0, window[1]), y1 = std::min(n, window[2]), x1 = std::min(n, window[3]);
+    const int blocks = (int)(((int64_t)n * n + kStaticPixelsPerBlock - 1) / kStaticPixelsPerBlock);    // <= kStaticMaxParts
+    hogbom_static_reset_kernel<<<1, 1, 0, st>>>(ctrl, (y1 <= y0 || x1 <= x0 || n_iter <= 0) ? 1 : 0);
+    psf_sidelobe_kernel<<<blocks, kCleanThreads, 0, st>>>(psf, n, ctrl);
+    for (int it = 0; it <= n_iter; ++it) {
+        hogbom_update_kernel<<<blocks, kCleanThreads, 0, st>>>(residual, psf, n, y0, x0, y1, x1, ctrl, part_val, part_idx);
+        hogbom_pick_kernel<<<1, kCleanThreads, 0, st>>>(residual, model, n, blocks, part_val, part_idx, gain, threshold,
+                                                        cycle_factor, it == n_iter, ctrl, components_out);
+    }
+    if (n_components_out) store_count_kernel<<<1, 1, 0, st>>>(ctrl, n_components_out);
+    IMAGER_CUDA(cudaGetLastError());
+    return 0;
 }
