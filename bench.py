@@ -29,7 +29,6 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 FP32_FMA_PER_CLK_SM = 128          # B200_PROFILING.md / SURVEY 8(d): 128 FP32 lanes per SM
-MEASURED_FFMA2_FMA_PER_CLK_SM = 113.3   # profiles/r1_port_probe.md: FFMA2 x16 at 0.565 clk per warp instruction per SM
 N_SM = 148
 
 
@@ -162,19 +161,21 @@ def workload_chunks(name, time_stride, chunk_steps):
     return [make_workload(name, time_stride=time_stride, time_range=(t0, t0 + chunk_steps)) for t0 in range(0, n_time, chunk_steps)]
 
 
-def dram_traffic_of_capture(workload, time_stride):
-    """DRAM bytes per launch of the gridding kernel from the committed `ncu --set full` capture -- used only if that
-    capture was taken on the kernel source that is being benchmarked (profiles/r2_traffic.txt carries its SHA-256)."""
+def counters_of_capture(workload, time_stride):
+    """Per-launch counters of the two hot kernels from the committed `ncu --set full` captures (profiles/r3_traffic.txt:
+    DRAM bytes read + written, wavefronts of the LSU data pipe) -- used only if the capture was taken on the kernel source that is being
+    benchmarked (the file carries the SHA-256 of gridder_tiled.cu) and on this workload at its full size."""
     import hashlib
-    prof = os.path.join(ROOT, "profiles", "r2_traffic.txt")
+    prof = os.path.join(ROOT, "profiles", "r3_traffic.txt")
     src = os.path.join(ROOT, "paper_2206_15117_b200", "csrc", "gridder_tiled.cu")
-    if not (os.path.exists(prof) and os.path.exists(src)) or workload != "config2" or time_stride != 1:
-        return None, "no capture for this workload"
+    if not (os.path.exists(prof) and os.path.exists(src)) or time_stride != 1:
+        return {}, "no capture for this workload"
     fields = dict(ln.split(None, 1) for ln in open(prof) if ln.strip() and not ln.startswith("#"))
     digest = hashlib.sha256(open(src, "rb").read()).hexdigest()
     if fields.get("gridder_tiled_cu_sha256", "").strip() != digest:
-        return None, "stale: the capture in profiles/r2_traffic.txt is of another version of gridder_tiled.cu"
-    return int(fields["grid_kernel_dram_bytes_per_launch"]), "profiles/r2_traffic.txt (ncu --set full, same kernel source)"
+        return {}, "stale: the captures in profiles/r3_traffic.txt are of another version of gridder_tiled.cu"
+    out = {k[len(workload) + 1:]: int(v) for k, v in fields.items() if k.startswith(workload + ".")}
+    return out, ("profiles/r3_traffic.txt (ncu --set full, same kernel source)" if out else "no capture for this workload")
 
 
 def run_ours(args):
@@ -197,6 +198,10 @@ def run_ours(args):
     multi = len(wls) > 1
     n, nc, npol = params["grid_size"], params["n_corr"], params["n_pol"]
     plan = Plan(params, max(w.nvis for w in wls))      # the library generates its own kernel tables (A0, untimed)
+    path, why = plan.path()
+    if path != "tiled" and not args.allow_reference:
+        raise SystemExit(f"bench.py: this plan would run on the library's reference kernels, not the tiled ones ({why}); "
+                         f"no line is printed for that path unless --allow-reference is given")
 
     # resident inputs, chunk by chunk
     def to_dev(w):
@@ -388,14 +393,26 @@ def run_ours(args):
     value = job_throughput(nvis, world, ms_per_step)
     sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
     peak_tflops = N_SM * FP32_FMA_PER_CLK_SM * sm_mhz * 1e6 * 2 / 1e12
-    peak_measured = N_SM * MEASURED_FFMA2_FMA_PER_CLK_SM * sm_mhz * 1e6 * 2 / 1e12
-    achieved = 8.0 * cmacs / (kern["grid"] * 1e-3) / 1e12
-    traffic, traffic_src = dram_traffic_of_capture(args.workload, args.time_stride)
+    # flop rates on EXECUTED complex MACs (8 flop each); the nominal count also holds the MACs of duplicate visibilities
+    # that the library pre-sums (same kernel set, cell and sub-cell: exact algebra, R16) and never executes
+    achieved = 8.0 * cmacs_exec / (kern["grid"] * 1e-3) / 1e12
+    achieved_nominal = 8.0 * cmacs / (kern["grid"] * 1e-3) / 1e12
+    achieved_d = 8.0 * cmacs_exec / (kern["degrid"] * 1e-3) / 1e12
+    achieved_d_nominal = 8.0 * cmacs / (kern["degrid"] * 1e-3) / 1e12
+    cap, traffic_src = counters_of_capture(args.workload, args.time_stride)
+    traffic, traffic_d = cap.get("grid.dram_bytes"), cap.get("degrid.dram_bytes")
+    # the unit that binds both kernels: the LSU data pipe passes one 128-byte wavefront per clock per SM
+    lsu_floor = lambda wavefronts: None if wavefronts is None else wavefronts / N_SM / (sm_mhz * 1e6) * 1e3
     in_bytes = nvis * (12 + 8 * nc + 4 * nc + (4 if wls[0].a_index is not None else 0))
     grid_bytes = npol * n * n * 8
     step_desc = ("imager_grid (index+sort+plan+grid) + imager_degrid (index reused)" if not multi else
                  f"{len(wls)} chunks of {args.chunk_steps} time steps through ONE plan: imager_grid per chunk (index+sort+plan+grid), "
                  f"then imager_degrid per chunk (index+sort+plan+degrid: the index of another chunk cannot be reused)")
+    peak_kind = f"148 SM x 128 FP32 lanes x 2 flop x {sm_mhz:.0f} MHz ({peaks_kind} max SM clock)"
+    dup_rate = stats["n_merged"] / max(1, stats["n_kept"])
+    mac_note = ("achieved / frac count EXECUTED complex MACs (8 flop each); *_nominal_incl_presummed also count the MACs of the "
+                "duplicate visibilities (same kernel set, cell and sub-cell) that the library sums before gridding and never "
+                "executes -- duplicate_rate = merged / kept visibilities says how much of the synthetic workload that is")
     line = {
         "metric": "visibilities gridded+degridded/sec", "value": value, "unit": "vis/s", "n_gpus": world,
         "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
@@ -403,6 +420,7 @@ def run_ours(args):
         "config": {"workload": args.workload, "nvis": nvis, "grid": n, "n_wplanes": params["n_wplanes"],
                    "support": [params["support_min"], params["support_max"]], "oversample": params["oversample"],
                    "n_corr": nc, "time_stride": args.time_stride, "chunks": len(wls), "parallelism": f"replicas x{world}",
+                   "kernel_path": path,
                    "l2": f"inputs ({in_bytes / 1e6:.0f} MB of visibilities + {grid_bytes / 1e6:.1f} MB grid) "
                          f"{'exceed' if in_bytes + grid_bytes > 126e6 else 'FIT IN'} the 126 MB L2; no explicit flush",
                    "step": step_desc, "e2e_step": e2e_desc},
@@ -412,23 +430,24 @@ def run_ours(args):
         "gpu_launches": launches,
         "roofline": {"bound": "alu", "kernel": "gridding (imager_grid, index reused)", "achieved": achieved,
                      "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": traffic,
-                     "traffic_source": traffic_src,
-                     "peak_kind": f"148 SM x 128 FP32 lanes x 2 flop x {sm_mhz:.0f} MHz ({peaks_kind} max SM clock)",
-                     "frac_of_measured_fma": achieved / peak_measured,
-                     "measured_fma_peak": peak_measured,
-                     "measured_fma_peak_kind": f"148 SM x {MEASURED_FFMA2_FMA_PER_CLK_SM} FMA/clk/SM (FFMA2 issue rate measured on "
-                                               f"this pool's B200: 0.565 clk per warp instruction per SM, profiles/r1_port_probe.md) x 2 flop x {sm_mhz:.0f} MHz",
+                     "traffic_source": traffic_src, "peak_kind": peak_kind,
+                     "lsu_wavefronts": cap.get("grid.lsu_wavefronts"), "lsu_floor_ms": lsu_floor(cap.get("grid.lsu_wavefronts")),
                      "kernel_ms": kern["grid"], "nominal_cmacs": cmacs, "executed_cmacs": cmacs_exec,
-                     "note": "achieved / frac count NOMINAL complex MACs (8 flop each: the algorithmic work of the pass); the kernel "
-                             "executes `executed_cmacs` (duplicate visibilities are pre-summed: exact algebra), frac_executed counts those",
-                     "frac_executed": 8.0 * cmacs_exec / (kern["grid"] * 1e-3) / 1e12 / peak_tflops,
-                     "merged_duplicates": stats["n_merged"], "hits": stats["n_hits"],
-                     "grid_vis_per_s": nvis / (kern["grid"] * 1e-3), "grid_cmac_per_s": cmacs / (kern["grid"] * 1e-3),
-                     "degrid_ms": kern["degrid"], "degrid_vis_per_s": nvis / (kern["degrid"] * 1e-3),
-                     "degrid_cmac_per_s": cmacs / (kern["degrid"] * 1e-3),
-                     "degrid_frac": 8.0 * cmacs / (kern["degrid"] * 1e-3) / 1e12 / peak_tflops,
+                     "achieved_nominal_incl_presummed": achieved_nominal,
+                     "frac_nominal_incl_presummed": achieved_nominal / peak_tflops,
+                     "merged_duplicates": stats["n_merged"], "duplicate_rate": dup_rate, "note": mac_note,
+                     "hits": stats["n_hits"],
+                     "grid_vis_per_s": nvis / (kern["grid"] * 1e-3), "grid_cmac_per_s": cmacs_exec / (kern["grid"] * 1e-3),
                      "cold_path_ms": ms_per_step - kern["grid"] - kern["degrid"],
                      "hbm_gbs_grid": (nvis * (16 + 4 + 8 * nc + 4 * nc) + 2 * grid_bytes) / (kern["grid"] * 1e-3) / 1e9},
+        "roofline_degrid": {"bound": "alu", "kernel": "degridding (imager_degrid, index reused)", "achieved": achieved_d,
+                            "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved_d / peak_tflops, "traffic": traffic_d,
+                            "traffic_source": traffic_src, "peak_kind": peak_kind,
+                            "lsu_wavefronts": cap.get("degrid.lsu_wavefronts"), "lsu_floor_ms": lsu_floor(cap.get("degrid.lsu_wavefronts")), "kernel_ms": kern["degrid"], "nominal_cmacs": cmacs,
+                            "executed_cmacs": cmacs_exec, "achieved_nominal_incl_presummed": achieved_d_nominal,
+                            "frac_nominal_incl_presummed": achieved_d_nominal / peak_tflops,
+                            "degrid_vis_per_s": nvis / (kern["degrid"] * 1e-3),
+                            "degrid_cmac_per_s": cmacs_exec / (kern["degrid"] * 1e-3)},
         "step_ms_all": step_ms,
     }
     if not args.no_cpu_baseline:
@@ -473,6 +492,7 @@ def main():
     ap.add_argument("--e2e-chunks", type=int, default=1, help="chunks of the end-to-end pipeline within a step (1 = one call per stage; steps are pipelined over two buffer sets either way)")
     ap.add_argument("--chunk-steps", type=int, default=100, help="config5: time steps per chunk fed through the API")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--allow-reference", action="store_true", help="print a line even if the plan runs on the library's slow reference kernels")
     args = ap.parse_args()
     if args.steps is None:
         args.steps = 5 if args.impl == "reference" else 50

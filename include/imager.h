@@ -163,8 +163,9 @@ int imager_mosaic_correct(imager_plan* plan, float* image, void* cuda_stream);
  * |psf| outside the 3 x 3 pixels at its centre; a = gain * residual[p]; model[p] += a; residual[q] -= a * psf[q - p + c]
  * wherever that psf sample exists.  Each step is one IEEE float32 operation (no fused multiply-add), so that peak positions
  * and component values are reproducible bit for bit.  components_out dev float32 [n_iter][3] = (y, x, a) in the order
- * found, or NULL; n_components_out dev int32 [1] or NULL.  Enqueues 2 n_iter + 3 kernels on cuda_stream; the stop test is
- * taken on the device, nothing is read back and nothing synchronises.  Errors: INVALID_ARG, NOMEM, CUDA. */
+ * found, or NULL; n_components_out dev int32 [1] or NULL.  Enqueues 2 n_iter + 3 kernels on cuda_stream (one more with
+ * n_components_out) whatever happens: the stop test is taken on the device, and once it has fired the launches still queued
+ * return at once (a few microseconds each: choose n_iter as a bound, not as a wish); nothing is read back and nothing synchronises.  Errors: INVALID_ARG, NOMEM, CUDA. */
 int imager_hogbom(float* residual, const float* psf, float* model, int32_t n, const int32_t window[4], float gain,
                   float threshold, float cycle_factor, int32_t n_iter, float* components_out, int32_t* n_components_out,
                   void* cuda_stream);
@@ -233,7 +234,8 @@ int imager_reproject(const float* src, int32_t n_src, double cell_src, float* ds
  * centre) is gridded on the plan's grid (imager_grid: index + bucket + grid), transformed (cuFFT + taper), weighted by the
  * Airy power beam of the plan (dish_diameter_m, freq_hz) and reprojected to the mosaic frame at offset pointing_lm[i];
  * mosaic_image = sum_i w_i B_i reproject_i[I_i], w_i = component i's sum of weights / the total.  `plan`: single
- * polarisation, one A-plane, kernel mode PSWF or WPROJ.  nvis host [n_point]; uvw, vis, weights host arrays of n_point DEVICE
+ * polarisation, one A-plane, kernel mode PSWF, WPROJ, DELTA or USER tables of that kind (a MOSAIC_PB or AWPROJ_* plan is refused
+ * with UNSUPPORTED: its kernels already hold the beam, which this call applies in the image plane).  nvis host [n_point]; uvw, vis, weights host arrays of n_point DEVICE
  * pointers ([nvis_i][3] float32, [nvis_i] complex64, [nvis_i] float32); pointing_lm host [n_point][2] radians;
  * mosaic_image dev complex64 [n_mosaic][n_mosaic] (OVERWRITTEN), cell_mosaic radians; sum_weights dev double [1] or NULL
  * (the total).  Synchronises once per component (its indexing step).  Errors: INVALID_ARG, UNSUPPORTED, TOO_MANY_VIS
@@ -265,9 +267,17 @@ int imager_debug_kernels(imager_plan* plan, int32_t kset, int32_t which, float* 
 
 /* info: [0] n_sets, [1] bucket tile size, [2] n_buckets, [3] key bits, [4] dropped visibilities of the last
  * indexing, [5] GPU kernel launches issued by the last imager_grid / imager_degrid call, [6] complex elements of one
- * table set collection, [7] kept visibilities of the last indexing.  [4] and [7] are read with a blocking copy on the
- * legacy default stream (it waits for work on that stream and on blocking streams, not for the whole device). */
+ * table set collection, [7] kept visibilities of the last indexing.  [4] and [7] are read back after waiting for the
+ * last indexing of this plan (an event recorded behind it on the stream it ran on, non-blocking streams included); no
+ * device-wide synchronisation. */
 int imager_plan_info(imager_plan* plan, int64_t info_out[8]);
+
+/* Which kernels imager_grid / imager_degrid will run for this plan (without IMAGER_PATH_REFERENCE): returns 1 for the tiled
+ * kernels (the fast path every number in bench.py is about), 0 for the one-warp-per-visibility reference kernels -- the
+ * library falls back to them, with the same results and several times the run time, for shapes the tiled kernels are not
+ * built for -- and then writes the reason into why_out (host char [why_len], NUL-terminated, "" when tiled; may be NULL
+ * with why_len 0).  Fixed at plan creation; no device work, no synchronisation.  < 0 on error (INVALID_ARG). */
+int imager_plan_path(imager_plan* plan, char* why_out, int32_t why_len);
 
 /* Statistics of the current index (built by the last imager_index / imager_grid / imager_degrid / imager_debug_index
  * call); synchronises cuda_stream.  out[0] kept visibilities, [1] dropped ones, [2] duplicates merged into another
@@ -290,6 +300,13 @@ int imager_last_launch_count(imager_plan* plan);
  * table, 7 window strip).  Returns 1 for a checked build, 0 for the normal build (out is zeroed), < 0 on error.
  * Synchronises the device. */
 int imager_debug_violations(int64_t out[16]);
+
+/* Micro-benchmarks of the two SM units that bound the gridding / degridding kernels, so that the numbers
+ * the design and bench.py's `lsu_floor_ms` rest on can be re-measured: out[0] clocks per warp-wide LDS.64 instruction per
+ * SM with all 32 lanes active, out[1] the same with 16 lanes active, out[2] clocks per warp-wide FFMA2 (fma.rn.f32x2)
+ * instruction per SM, out[3] the SM count.  Allocates and frees 4 KB of device memory, launches six small kernels (one
+ * 1024-thread CTA per SM, a few hundred microseconds), synchronises cuda_stream.  Errors: INVALID_ARG, NOMEM, CUDA. */
+int imager_debug_probe(double out[4], void* cuda_stream);
 
 /* Thread-local message of the last failing call on this thread ("" if none); valid until the next call. */
 const char* imager_last_error(void);

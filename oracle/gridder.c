@@ -34,6 +34,12 @@ static inline int64_t tap_index(int n_corr, int O, int S, int s, int c, int oy, 
     return (((((int64_t)s * n_corr + c) * O + oy) * O + ox) * S + dy) * S + dx;
 }
 
+/* Reading R24 (extends R9 "omega = 0 contributes 0"): sample j = (visibility, correlation) is FLAGGED when its
+ * weight is zero or its weight or value is not finite; a flagged sample contributes (0, 0) and no weight. */
+static int sample_flagged(const float* weights, const float* vis, int64_t j) {
+    return weights[j] == 0.0f || !isfinite(weights[j]) || !isfinite(vis[2 * j]) || !isfinite(vis[2 * j + 1]);
+}
+
 /* O4.  grid, norm: [n_pol][N][N] (grid as interleaved re,im doubles), accumulated into.
  * If sample_rowptr != NULL only the listed cells are computed: sample_rowptr[N+1] is a CSR over rows of
  * sample_x (sorted), and outputs are written to sample_out[n_pol][n_samples] (re,im) / sample_norm instead. */
@@ -67,6 +73,7 @@ int oracle_grid(int64_t nvis, int N, int n_corr, int n_pol, int O,
                 const double w = (double)weights[k * n_corr + c];
                 vr[c] = w * (double)vis[2 * (k * n_corr + c)];
                 vi[c] = w * (double)vis[2 * (k * n_corr + c) + 1];
+                if (sample_flagged(weights, vis, k * n_corr + c)) vr[c] = vi[c] = 0.0;   /* R24 */
                 va[c] = hypot(vr[c], vi[c]);
             }
             for (int dy = 0; dy < S; ++dy) {
@@ -114,7 +121,8 @@ int oracle_grid(int64_t nvis, int N, int n_corr, int n_pol, int O,
     }
     for (int64_t k = 0; k < nvis; ++k)                              /* dropped visibilities carry no weight (R8) */
         if (!drop[k])
-            for (int c = 0; c < n_corr; ++c) sumwt[c] += (double)weights[k * n_corr + c];
+            for (int c = 0; c < n_corr; ++c)
+                if (!sample_flagged(weights, vis, k * n_corr + c)) sumwt[c] += (double)weights[k * n_corr + c];   /* R24 */
     return 0;
 }
 

@@ -21,10 +21,10 @@ PATH_REFERENCE = 2
 DEGRID_RESIDUAL = 16
 
 EXPORTS = ("imager_plan_create", "imager_index", "imager_grid", "imager_degrid", "imager_plan_destroy",
-           "imager_grid_image_transform", "imager_mosaic_correct", "imager_debug_index", "imager_debug_kernels", "imager_plan_info",
+           "imager_grid_image_transform", "imager_mosaic_correct", "imager_debug_index", "imager_debug_kernels", "imager_plan_info", "imager_plan_path",
            "imager_index_stats", "imager_hogbom", "imager_hogbom_static", "imager_clean", "imager_reproject", "imager_mosaic_grid",
            "imager_mosaic_degrid",
-           "imager_last_launch_count", "imager_debug_violations", "imager_last_error")
+           "imager_last_launch_count", "imager_debug_violations", "imager_debug_probe", "imager_last_error")
 
 
 class ImagerError(RuntimeError):
@@ -68,6 +68,7 @@ def load_library() -> ctypes.CDLL:
                                        POINTER(c_int64), c_void_p]
     lib.imager_debug_kernels.argtypes = [c_void_p, c_int32, c_int32, c_void_p, POINTER(c_int32)]
     lib.imager_plan_info.argtypes = [c_void_p, POINTER(c_int64)]
+    lib.imager_plan_path.argtypes = [c_void_p, c_char_p, c_int32]
     lib.imager_index_stats.argtypes = [c_void_p, POINTER(c_int64), c_void_p]
     lib.imager_reproject.argtypes = [c_void_p, c_int32, c_double, c_void_p, c_int32, c_double, c_double, c_double, c_int32,
                                      c_double, c_double, c_int32, c_int32, c_void_p]
@@ -82,6 +83,7 @@ def load_library() -> ctypes.CDLL:
                                  c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]
     lib.imager_last_launch_count.argtypes = [c_void_p]
     lib.imager_debug_violations.argtypes = [POINTER(c_int64)]
+    lib.imager_debug_probe.argtypes = [POINTER(c_double), c_void_p]
     _lib = lib
     return lib
 
@@ -255,6 +257,14 @@ class Plan:
         names = ("n_sets", "bucket_tile", "n_buckets", "key_bits", "n_dropped", "last_launches", "table_elems", "n_kept")
         return dict(zip(names, [int(x) for x in out]))
 
+    def path(self) -> tuple[str, str]:
+        """imager_plan_path: ("tiled", "") or ("reference", why the tiled kernels cannot run this plan)."""
+        buf = ctypes.create_string_buffer(256)
+        rc = load_library().imager_plan_path(self._h, buf, len(buf))
+        if rc < 0:
+            _check(rc, "imager_plan_path")
+        return ("tiled" if rc == 1 else "reference", buf.value.decode())
+
     def index_stats(self, stream=None) -> dict:
         out = (c_int64 * 8)()
         _check(load_library().imager_index_stats(self._h, out, _stream_ptr(stream)), "imager_index_stats")
@@ -296,6 +306,13 @@ def hogbom(residual, psf, model, window, gain: float, threshold: float, cycle_fa
         _dev_ptr(residual, torch.float32, "residual"), _dev_ptr(psf, torch.float32, "psf"), _dev_ptr(model, torch.float32, "model"),
         n, win, float(gain), float(threshold), float(cycle_factor), int(n_iter), _dev_ptr(components_out, torch.float32, "components_out"),
         _dev_ptr(n_components_out, torch.int32, "n_components_out"), _stream_ptr(stream)), "imager_hogbom")
+
+
+def debug_probe(stream=None) -> dict:
+    """imager_debug_probe: clocks per warp instruction per SM of LDS.64 (32 and 16 active lanes) and FFMA2."""
+    out = (c_double * 4)()
+    _check(load_library().imager_debug_probe(out, _stream_ptr(stream)), "imager_debug_probe")
+    return {"lds64_clk": out[0], "lds64_half_mask_clk": out[1], "ffma2_clk": out[2], "n_sm": int(out[3])}
 
 
 HOGBOM_STATIC_MAX_N = 4096

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libimager.so")
 LIB_CHECKED = os.path.join(HERE, "libimager_checked.so")   # -DIMAGER_CHECKED=1: device-side bounds checks (include/imager.h)
-SOURCES = ["api.cu", "index_sort.cu", "gridder_ref.cu", "gridder_tiled.cu", "tables.cu", "transform.cu", "clean.cu", "mosaic.cu"]
+SOURCES = ["api.cu", "index_sort.cu", "gridder_ref.cu", "gridder_tiled.cu", "tables.cu", "transform.cu", "clean.cu", "mosaic.cu", "probe.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC",
               "-Xptxas", "-v"]
 

@@ -16,6 +16,18 @@ void set_error(const char* fmt, ...) {
     va_end(ap);
 }
 
+int num_sms() {
+    static int cached[64] = {};                      // per device ordinal; a B200 has 148
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
+    if (!cached[dev]) {
+        int n = 0;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+        cached[dev] = n;
+    }
+    return cached[dev];
+}
+
 int cuda_fail(cudaError_t e, const char* what) {
     set_error("CUDA error %d (%s) in %s", (int)e, cudaGetErrorString(e), what);
     return e == cudaErrorMemoryAllocation ? IMAGER_ERR_NOMEM : IMAGER_ERR_CUDA;
@@ -54,6 +66,7 @@ static int check_params(const imager_params* p) {
 
 static void free_plan(imager_plan* pl) {
     if (!pl) return;
+    if (pl->index_done) cudaEventDestroy(pl->index_done);
     if (pl->d_tab_degrid && pl->d_tab_degrid != pl->d_tab_grid) cudaFree(pl->d_tab_degrid);
     cudaFree(pl->d_tab_grid);
     cudaFree(pl->d_set_offset);
@@ -155,6 +168,7 @@ extern "C" int imager_plan_create(const imager_params* params, void* cuda_stream
     PLAN_CUDA(cudaMemsetAsync(pl->d_counters, 0, 64 * sizeof(int32_t), st));
     pl->max_items = (int64_t)pl->n_sets * pl->nt * pl->nt;
     PLAN_CUDA(cudaMalloc(&pl->d_items, (pl->max_items + 1) * 4 * sizeof(int32_t)));
+    PLAN_CUDA(cudaEventCreateWithFlags(&pl->index_done, cudaEventDisableTiming));
     PLAN_CUDA(cudaStreamSynchronize(st));
 #undef PLAN_CUDA
     rc = build_tables(pl, params, st);
@@ -174,7 +188,9 @@ static int ensure_index(imager_plan* pl, int64_t nvis, const float* uvw, const i
     if (nvis > pl->p.max_nvis) { set_error("nvis exceeds max_nvis"); return IMAGER_ERR_TOO_MANY_VIS; }
     if ((flags & IMAGER_REUSE_INDEX) && pl->index_valid && pl->indexed_nvis == nvis) return 0;
     if (nvis > 0 && !uvw) { set_error("uvw is NULL"); return IMAGER_ERR_INVALID_ARG; }
-    return run_index_and_sort(pl, nvis, uvw, a_index, st);
+    const int rc = run_index_and_sort(pl, nvis, uvw, a_index, st);
+    if (rc == 0 && pl->index_done) IMAGER_CUDA(cudaEventRecord(pl->index_done, st));
+    return rc;
 }
 
 extern "C" int imager_index(imager_plan* plan, int64_t nvis, const float* uvw, const int32_t* a_index, void* cuda_stream) {
@@ -195,7 +211,7 @@ extern "C" int imager_grid(imager_plan* plan, int64_t nvis, const float* uvw, co
     plan->last_launches = 0;
     int rc = ensure_index(plan, nvis, uvw, a_index, flags, st);
     if (rc) return rc;
-    rc = launch_sum_weights(plan, nvis, weights, sum_weights, st);
+    rc = launch_sum_weights(plan, nvis, (const float2*)vis, weights, sum_weights, st);
     if (rc) return rc;
     if (!(flags & IMAGER_PATH_REFERENCE) && tiled_supported(plan))
         return launch_grid_tiled(plan, nvis, (const float2*)vis, weights, (float2*)grid, st);
@@ -283,11 +299,22 @@ extern "C" int imager_last_launch_count(imager_plan* plan) {
     return plan ? plan->last_launches : (int)IMAGER_ERR_INVALID_ARG;
 }
 
+extern "C" int imager_plan_path(imager_plan* plan, char* why_out, int32_t why_len) {
+    g_err[0] = 0;
+    if (!plan || why_len < 0 || (why_len > 0 && !why_out)) { set_error("NULL argument"); return IMAGER_ERR_INVALID_ARG; }
+    const char* why = tiled_unsupported_reason(plan);
+    if (why_len > 0) snprintf(why_out, (size_t)why_len, "%s", why ? why : "");
+    return why ? 0 : 1;
+}
+
 extern "C" int imager_plan_info(imager_plan* plan, int64_t info_out[8]) {
     g_err[0] = 0;
     if (!plan || !info_out) { set_error("NULL argument"); return IMAGER_ERR_INVALID_ARG; }
     int32_t c[2] = {0, 0};
-    IMAGER_CUDA(cudaMemcpy(c, plan->d_counters, sizeof(c), cudaMemcpyDeviceToHost));     // blocking copy on the legacy stream
+    // the counters are written by the last indexing, on whatever stream that ran (possibly a non-blocking one, which the
+    // legacy-stream copy below would not wait for): wait for the event recorded behind it first
+    if (plan->index_done) IMAGER_CUDA(cudaEventSynchronize(plan->index_done));
+    IMAGER_CUDA(cudaMemcpy(c, plan->d_counters, sizeof(c), cudaMemcpyDeviceToHost));
     info_out[0] = plan->n_sets;
     info_out[1] = kBucketTile;
     info_out[2] = plan->n_buckets;

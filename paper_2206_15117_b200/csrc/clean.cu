@@ -151,17 +151,24 @@ __global__ void store_count_kernel(const HogbomCtrl* __restrict__ ctrl, int32_t*
 int run_hogbom(float* residual, const float* psf, float* model, int n, const int32_t window[4], float gain, float threshold,
                float cycle_factor, int n_iter, float* components_out, int32_t* n_components_out, cudaStream_t st, int* launches) {
     const int y0 = std::max(0, window[0]), x0 = std::max(0, window[1]), y1 = std::min(n, window[2]), x1 = std::min(n, window[3]);
-    const int blocks = (int)std::min<int64_t>(((int64_t)n * n + kCleanThreads - 1) / kCleanThreads, 4 * kNumSMs);
+    const int blocks = (int)std::min<int64_t>(((int64_t)n * n + kCleanThreads - 1) / kCleanThreads, 4 * num_sms());
     HogbomCtrl* ctrl = nullptr;
     float* part_val = nullptr;
     int32_t* part_idx = nullptr;
-    IMAGER_CUDA(cudaMallocAsync(&ctrl, sizeof(HogbomCtrl), st));
-    IMAGER_CUDA(cudaMallocAsync(&part_val, blocks * sizeof(float), st));
-    IMAGER_CUDA(cudaMallocAsync(&part_idx, blocks * sizeof(int32_t), st));
+    auto fail = [&](cudaError_t e, const char* what) {      // an exit on error frees what was allocated so far
+        if (ctrl) cudaFreeAsync(ctrl, st);
+        if (part_val) cudaFreeAsync(part_val, st);
+        if (part_idx) cudaFreeAsync(part_idx, st);
+        return cuda_fail(e, what);
+    };
+#define HOGBOM_CUDA(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return fail(e__, #call); } while (0)
+    HOGBOM_CUDA(cudaMallocAsync(&ctrl, sizeof(HogbomCtrl), st));
+    HOGBOM_CUDA(cudaMallocAsync(&part_val, blocks * sizeof(float), st));
+    HOGBOM_CUDA(cudaMallocAsync(&part_idx, blocks * sizeof(int32_t), st));
     HogbomCtrl init = {};
     init.p = -1;
     if (y1 <= y0 || x1 <= x0 || n_iter <= 0) init.done = 1;
-    IMAGER_CUDA(cudaMemcpyAsync(ctrl, &init, sizeof(init), cudaMemcpyHostToDevice, st));   // pageable source: copied before return
+    HOGBOM_CUDA(cudaMemcpyAsync(ctrl, &init, sizeof(init), cudaMemcpyHostToDevice, st));   // pageable source: copied before return
     psf_sidelobe_kernel<<<blocks, kCleanThreads, 0, st>>>(psf, n, ctrl);
     int count = 1;
     for (int it = 0; it <= n_iter; ++it) {
@@ -174,7 +181,8 @@ int run_hogbom(float* residual, const float* psf, float* model, int n, const int
         store_count_kernel<<<1, 1, 0, st>>>(ctrl, n_components_out);
         ++count;
     }
-    IMAGER_CUDA(cudaGetLastError());
+    HOGBOM_CUDA(cudaGetLastError());
+#undef HOGBOM_CUDA
     IMAGER_CUDA(cudaFreeAsync(ctrl, st));
     IMAGER_CUDA(cudaFreeAsync(part_val, st));
     IMAGER_CUDA(cudaFreeAsync(part_idx, st));
@@ -232,7 +240,7 @@ extern "C" int imager_clean(imager_plan* plan, int64_t nvis, const float* uvw, c
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int n = plan->p.grid_size;
     const int64_t npix = (int64_t)n * n;
-    const unsigned gb = 4 * kNumSMs;
+    const unsigned gb = 4 * num_sms();
     float2* work = nullptr;                      // [N][N] complex: grid <-> image
     float *psf = nullptr, *cycle = nullptr;
     double* sumwt = nullptr;

@@ -12,8 +12,8 @@ namespace imager {
 constexpr int kBucketTile = 32;          // bucketing tile (cells); DESIGN.md "Bucketing key"
 constexpr uint32_t kKeyDrop = 0xFFFFFFFFu;   // exported key of a dropped visibility (the oracle's KEY_DROP)
 constexpr int kSortChunk = 4096;         // items per CTA tile in the radix sort
-constexpr int kNumSMs = 148;             // B200
 
+int num_sms();                           // SMs of the current device (cudaDevAttrMultiProcessorCount, cached per device): launch sizes
 void set_error(const char* fmt, ...);
 int cuda_fail(cudaError_t e, const char* what);
 
@@ -22,6 +22,16 @@ int cuda_fail(cudaError_t e, const char* what);
         cudaError_t e__ = (call);                                      \
         if (e__ != cudaSuccess) return ::imager::cuda_fail(e__, #call); \
     } while (0)
+
+// R24: a sample (visibility k, correlation c) with zero weight, or with a weight or value that is not finite, is
+// FLAGGED: it contributes (0, 0) to the grid and nothing to the sum of weights -- flagged data often carry NaN, and
+// 0 * NaN would otherwise poison every cell of the footprint (and, in the tiled kernel, the padding around it).
+__device__ __forceinline__ bool sample_flagged(float w, float2 v) {
+    return w == 0.f || !isfinite(w) || !isfinite(v.x) || !isfinite(v.y);
+}
+__device__ __forceinline__ float2 weighted_sample(float w, float2 v) {
+    return sample_flagged(w, v) ? make_float2(0.f, 0.f) : make_float2(w * v.x, w * v.y);
+}
 
 }  // namespace imager
 
@@ -65,6 +75,8 @@ struct imager_plan {
     void* fft_plan = nullptr;            // cufftHandle stored as intptr
     bool fft_ready = false;
 
+    cudaEvent_t index_done = nullptr;    // recorded behind every (re)indexing, on the stream it ran on: imager_plan_info waits for it
+
     int last_launches = 0;
 };
 
@@ -81,10 +93,11 @@ int launch_grid_reference(imager_plan* pl, int64_t nvis, const float2* vis, cons
                           const int32_t* set_mask, cudaStream_t st);
 int launch_degrid_reference(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, const int32_t* set_mask,
                             int residual, cudaStream_t st);
-int launch_sum_weights(imager_plan* pl, int64_t nvis, const float* weights, double* sum_weights, cudaStream_t st);
+int launch_sum_weights(imager_plan* pl, int64_t nvis, const float2* vis, const float* weights, double* sum_weights, cudaStream_t st);
 
 // gridder_tiled.cu
 bool tiled_supported(const imager_plan* pl);
+const char* tiled_unsupported_reason(const imager_plan* pl);   // NULL = supported
 int launch_grid_tiled(imager_plan* pl, int64_t nvis, const float2* vis, const float* weights, float2* grid,
                       cudaStream_t st);
 int launch_degrid_tiled(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, int residual, cudaStream_t st);

@@ -31,7 +31,7 @@ grid_ref_kernel(const int32_t* __restrict__ counters, const int32_t* __restrict_
         for (int c = 0; c < NC; ++c) {
             const float2 v = vis[(int64_t)k * NC + c];
             const float w = weights[(int64_t)k * NC + c];
-            val[c] = make_float2(w * v.x, w * v.y);
+            val[c] = weighted_sample(w, v);                                  // R24
         }
         const float2* T = tab + set_offset[r.kset] + (int64_t)sub * SS;
         const int64_t elem_stride = (int64_t)O * O * SS;
@@ -113,7 +113,7 @@ degrid_ref_kernel(int64_t nvis, const imager_record* __restrict__ rec, const int
 }
 
 template <int NC>
-__global__ void sum_weights_kernel(int64_t nvis, const imager_record* __restrict__ rec,
+__global__ void sum_weights_kernel(int64_t nvis, const imager_record* __restrict__ rec, const float2* __restrict__ vis,
                                    const float* __restrict__ weights, double* __restrict__ sum_weights) {
     double acc[NC];
 #pragma unroll
@@ -121,7 +121,10 @@ __global__ void sum_weights_kernel(int64_t nvis, const imager_record* __restrict
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < nvis; k += (int64_t)gridDim.x * blockDim.x) {
         if ((rec[k].sub >> 16) & 1u) continue;
 #pragma unroll
-        for (int c = 0; c < NC; ++c) acc[c] += (double)weights[k * NC + c];
+        for (int c = 0; c < NC; ++c) {
+            const float w = weights[k * NC + c];
+            if (!sample_flagged(w, vis[k * NC + c])) acc[c] += (double)w;           // R24: a flagged sample carries no weight
+        }
     }
 #pragma unroll
     for (int c = 0; c < NC; ++c) {
@@ -131,11 +134,11 @@ __global__ void sum_weights_kernel(int64_t nvis, const imager_record* __restrict
     }
 }
 
-int launch_sum_weights(imager_plan* pl, int64_t nvis, const float* weights, double* sum_weights, cudaStream_t st) {
+int launch_sum_weights(imager_plan* pl, int64_t nvis, const float2* vis, const float* weights, double* sum_weights, cudaStream_t st) {
     if (!sum_weights || nvis == 0) return 0;
-    const unsigned blocks = (unsigned)std::min<int64_t>((nvis + 255) / 256, 4 * kNumSMs);
-    if (pl->p.n_corr == 1) sum_weights_kernel<1><<<blocks, 256, 0, st>>>(nvis, pl->d_rec, weights, sum_weights);
-    else sum_weights_kernel<4><<<blocks, 256, 0, st>>>(nvis, pl->d_rec, weights, sum_weights);
+    const unsigned blocks = (unsigned)std::min<int64_t>((nvis + 255) / 256, 4 * num_sms());
+    if (pl->p.n_corr == 1) sum_weights_kernel<1><<<blocks, 256, 0, st>>>(nvis, pl->d_rec, vis, weights, sum_weights);
+    else sum_weights_kernel<4><<<blocks, 256, 0, st>>>(nvis, pl->d_rec, vis, weights, sum_weights);
     pl->last_launches++;
     IMAGER_CUDA(cudaGetLastError());
     return 0;
@@ -144,7 +147,7 @@ int launch_sum_weights(imager_plan* pl, int64_t nvis, const float* weights, doub
 int launch_grid_reference(imager_plan* pl, int64_t nvis, const float2* vis, const float* weights, float2* grid,
                           const int32_t* set_mask, cudaStream_t st) {
     if (nvis == 0) return 0;
-    const unsigned blocks = (unsigned)std::min<int64_t>((nvis + 7) / 8, 16 * kNumSMs);
+    const unsigned blocks = (unsigned)std::min<int64_t>((nvis + 7) / 8, 16 * num_sms());
     const int N = pl->p.grid_size, O = pl->p.oversample;
     if (pl->p.n_corr == 1)
         grid_ref_kernel<1, 1><<<blocks, 256, 0, st>>>(pl->d_counters, pl->d_perm[pl->sorted_buf], pl->d_rec, vis, weights,
@@ -160,7 +163,7 @@ int launch_grid_reference(imager_plan* pl, int64_t nvis, const float2* vis, cons
 int launch_degrid_reference(imager_plan* pl, int64_t nvis, const float2* grid, float2* vis_out, const int32_t* set_mask,
                             int residual, cudaStream_t st) {
     if (nvis == 0) return 0;
-    const unsigned blocks = (unsigned)std::min<int64_t>((nvis + 7) / 8, 16 * kNumSMs);
+    const unsigned blocks = (unsigned)std::min<int64_t>((nvis + 7) / 8, 16 * num_sms());
     const int N = pl->p.grid_size, O = pl->p.oversample;
     if (pl->p.n_corr == 1)
         degrid_ref_kernel<1, 1><<<blocks, 256, 0, st>>>(nvis, pl->d_rec, pl->d_perm[pl->sorted_buf], grid, pl->d_tab_degrid,

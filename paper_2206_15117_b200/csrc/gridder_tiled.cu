@@ -193,7 +193,7 @@ __global__ void gather_values_kernel(const int32_t* __restrict__ counters, const
         for (int c = 0; c < NC; ++c) {
             const float2 v = vis[k * NC + c];
             const float w = weights[k * NC + c];
-            sval[(int64_t)i * NC + c] = make_float2(w * v.x, w * v.y);
+            sval[(int64_t)i * NC + c] = weighted_sample(w, v);                  // R24
         }
     }
 }
@@ -217,7 +217,7 @@ __global__ void __launch_bounds__(1024) gather_merge_values_kernel(const int32_t
         for (int c = 0; c < NC; ++c) {
             const float2 v = vis[k * NC + c];
             const float w = weights[k * NC + c];
-            s_val[(i - c0) * NC + c] = make_float2(w * v.x, w * v.y);
+            s_val[(i - c0) * NC + c] = weighted_sample(w, v);                // R24
         }
     }
     __syncthreads();
@@ -1120,9 +1120,12 @@ static int table_pitch(int S) {
     return ((S + 2 * kPadX + 7) / 16) * 16 + 8;
 }
 
-bool tiled_supported(const imager_plan* pl) {
+// NULL if the tiled kernels can run this plan, else the reason they cannot (imager_plan_path reports it)
+const char* tiled_unsupported_reason(const imager_plan* pl) {
     const imager_params& p = pl->p;
-    if (p.grid_size % kStripH != 0 || p.grid_size > 32768 || pl->n_sets >= (1 << (32 - kSubBits))) return false;
+    if (p.grid_size % kStripH != 0) return "grid_size is not a multiple of the 32-cell strip height";
+    if (p.grid_size > 32768) return "grid_size exceeds 32768";
+    if (pl->n_sets >= (1 << (32 - kSubBits))) return "too many kernel sets for the hit record's set field";
     // every slice (with its padding) must fit in shared memory, and the planner enumerates (gu, strip) pairs
     const int64_t n_strips = (int64_t)(p.grid_size / kStripW) * (p.grid_size / kStripH);
     int64_t n_gu = 0;
@@ -1130,14 +1133,17 @@ bool tiled_supported(const imager_plan* pl) {
         const int S = pl->set_support[k];
         const int pitch = table_pitch(S);
         const int64_t slice_bytes = (int64_t)(S + 2 * kPadY) * pitch * 8;
-        if (slice_bytes > kTableBudget) return false;
+        if (slice_bytes > kTableBudget) return "one sub-cell slice of the largest kernel exceeds the shared-memory table budget";
         int gs = p.oversample * p.oversample;
         while (gs > 1 && gs * slice_bytes > kTableBudget) gs >>= 1;
-        if ((p.oversample * p.oversample) % gs) return false;
+        if ((p.oversample * p.oversample) % gs) return "oversample^2 is not a multiple of the sub-cell group size";
         n_gu += (p.oversample * p.oversample) / gs;
     }
-    return n_gu * n_strips <= kMaxPlanCells;
+    if (n_gu * n_strips > kMaxPlanCells) return "(kernel slice group, strip) pairs exceed the planner's table";
+    return nullptr;
 }
+
+bool tiled_supported(const imager_plan* pl) { return tiled_unsupported_reason(pl) == nullptr; }
 
 static TiledState* state_of(imager_plan* pl) {
     if (pl->tiled) return static_cast<TiledState*>(pl->tiled);
@@ -1278,7 +1284,7 @@ static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
     sorted_geo_dedupe_kernel<<<(unsigned)((pl->indexed_nvis + kDedupeChunk - 1) / kDedupeChunk), kDedupeThreads, kDedupeSmem, stream>>>(
         pl->d_counters, pl->d_perm[pl->sorted_buf], pl->d_rec, pl->p.oversample, st->d_sgeo, st->d_rep);
 #else
-    sorted_geo_kernel<<<4 * kNumSMs, 256, 0, stream>>>(pl->d_counters, pl->d_perm[pl->sorted_buf], pl->d_rec,
+    sorted_geo_kernel<<<4 * num_sms(), 256, 0, stream>>>(pl->d_counters, pl->d_perm[pl->sorted_buf], pl->d_rec,
                                                        pl->p.oversample, st->d_sgeo);
 #endif
     PlanArgs pa;
@@ -1290,8 +1296,8 @@ static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
     pa.cap_hits = 0;
     IMAGER_CUDA(cudaMemsetAsync(st->d_hits, 0, (n_cells + 1) * sizeof(int32_t), stream));
     IMAGER_CUDA(cudaMemsetAsync(st->d_total, 0, sizeof(unsigned long long), stream));
-    count_hits_kernel<<<8 * kNumSMs, 256, 0, stream>>>(pa, pl->d_counters, st->d_hits, st->d_total);
-    items_from_hits_kernel<<<2 * kNumSMs, 256, 0, stream>>>(n_cells, st->d_hits, st->d_items);
+    count_hits_kernel<<<8 * num_sms(), 256, 0, stream>>>(pa, pl->d_counters, st->d_hits, st->d_total);
+    items_from_hits_kernel<<<2 * num_sms(), 256, 0, stream>>>(n_cells, st->d_hits, st->d_items);
     pl->last_launches += 3;
     int rc = exclusive_scan_i32(pl, st->d_hits, n_cells + 1, st->d_scan_tmp, stream);
     if (rc) return rc;
@@ -1326,8 +1332,8 @@ static int prepare(imager_plan* pl, TiledState* st, cudaStream_t stream) {
     rc = grow(&st->d_hit_tmp, &st->cap_tmp, n_hits + 1);
     if (rc) return rc;
     IMAGER_CUDA(cudaMemsetAsync(st->d_cursor, 0, (n_cells + 1) * sizeof(int32_t), stream));
-    emit_hits_kernel<<<8 * kNumSMs, 256, 0, stream>>>(pa, pl->d_counters, st->d_hits, st->d_cursor, st->d_hit_tmp);
-    make_items_kernel<<<8 * kNumSMs, 256, 0, stream>>>(g, st->d_hits, st->d_items, st->d_item_rec);
+    emit_hits_kernel<<<8 * num_sms(), 256, 0, stream>>>(pa, pl->d_counters, st->d_hits, st->d_cursor, st->d_hit_tmp);
+    make_items_kernel<<<8 * num_sms(), 256, 0, stream>>>(g, st->d_hits, st->d_items, st->d_item_rec);
     if (n_items > 0)
         sort_items_kernel<<<(unsigned)((n_items + 7) / 8), 256, 0, stream>>>((int)n_items, st->d_item_rec, st->d_hit_tmp,
                                                                              st->d_hit_rec);
@@ -1395,7 +1401,7 @@ int tiled_index_stats(imager_plan* pl, int64_t out[8], cudaStream_t stream) {
     unsigned long long h[3] = {0, 0, 0};
     int32_t c[2] = {0, 0};
     if (e == cudaSuccess) {
-        index_stats_kernel<<<4 * kNumSMs, 256, 0, stream>>>(pl->d_counters, pl->d_perm[pl->sorted_buf], pl->d_rec,
+        index_stats_kernel<<<4 * num_sms(), 256, 0, stream>>>(pl->d_counters, pl->d_perm[pl->sorted_buf], pl->d_rec,
                                                             pl->d_set_support, planned ? st->d_sgeo : nullptr, d_out);
         e = cudaMemcpyAsync(h, d_out, sizeof(h), cudaMemcpyDeviceToHost, stream);
     }
@@ -1427,7 +1433,7 @@ int launch_grid_tiled(imager_plan* pl, int64_t nvis, const float2* vis, const fl
     TiledState* st = state_of(pl);
     int rc = prepare(pl, st, stream);
     if (rc) return rc;
-    const unsigned gb = 4 * kNumSMs;
+    const unsigned gb = 4 * num_sms();
     if (st->d_rep) {                          // duplicates pre-summed: gather and merge in one pass over the dedupe chunks
         const unsigned chunks = (unsigned)((pl->indexed_nvis + kDedupeChunk - 1) / kDedupeChunk);
         if (pl->p.n_corr == 1)
@@ -1445,9 +1451,9 @@ int launch_grid_tiled(imager_plan* pl, int64_t nvis, const float2* vis, const fl
     TiledArgs a;
     fill_args(pl, st, a, pl->d_tab_grid);
     if (pl->p.n_corr == 1)
-        grid_tiled_kernel<1><<<kNumSMs, kGridThreads, st->smem_bytes + kGridStageBytes, stream>>>(a, st->d_sval, grid);
+        grid_tiled_kernel<1><<<num_sms(), kGridThreads, st->smem_bytes + kGridStageBytes, stream>>>(a, st->d_sval, grid);
     else
-        grid_tiled_kernel<4><<<kNumSMs, kGridThreads, st->smem_bytes + kGridStageBytes, stream>>>(a, st->d_sval, grid);
+        grid_tiled_kernel<4><<<num_sms(), kGridThreads, st->smem_bytes + kGridStageBytes, stream>>>(a, st->d_sval, grid);
     pl->last_launches += 2;
     IMAGER_CUDA(cudaGetLastError());
     return 0;
@@ -1464,12 +1470,12 @@ int launch_degrid_tiled(imager_plan* pl, int64_t nvis, const float2* grid, float
     TiledArgs a;
     fill_args(pl, st, a, pl->d_tab_degrid);
     const int smem = st->smem_bytes + kStageBytes + kRedBytes;
-    const unsigned gb = 4 * kNumSMs;
+    const unsigned gb = 4 * num_sms();
     if (nc == 1) {
-        degrid_tiled_kernel<1><<<kNumSMs, kTiledThreads, smem, stream>>>(a, grid, st->d_sval);
+        degrid_tiled_kernel<1><<<num_sms(), kTiledThreads, smem, stream>>>(a, grid, st->d_sval);
         scatter_values_kernel<1><<<gb, 256, 0, stream>>>(nvis, pl->d_counters, pl->d_perm[pl->sorted_buf], st->d_rep, st->d_sval, residual, vis_out);
     } else {
-        degrid_tiled_kernel<4><<<kNumSMs, kTiledThreads, smem, stream>>>(a, grid, st->d_sval);
+        degrid_tiled_kernel<4><<<num_sms(), kTiledThreads, smem, stream>>>(a, grid, st->d_sval);
         scatter_values_kernel<4><<<gb, 256, 0, stream>>>(nvis, pl->d_counters, pl->d_perm[pl->sorted_buf], st->d_rep, st->d_sval, residual, vis_out);
     }
     pl->last_launches += 2;

@@ -99,6 +99,13 @@ static int check_mosaic_args(imager_plan* plan, int32_t n_point, const int64_t* 
         set_error("image-domain mosaic needs a single-polarisation component plan with one A-plane");
         return IMAGER_ERR_UNSUPPORTED;
     }
+    const int mode = plan->p.kernel_mode;
+    if (mode == IMAGER_MODE_MOSAIC_PB || mode == IMAGER_MODE_AWPROJ_ADJOINT || mode == IMAGER_MODE_AWPROJ_PAPER) {
+        // the beam is applied here, in the image plane (reproject): a plan whose gridding kernel already holds it would apply it twice
+        set_error("image-domain mosaic needs a plan WITHOUT a beam in its kernels (PSWF, WPROJ, or USER tables of that kind); "
+                  "kernel_mode %d carries the primary beam", mode);
+        return IMAGER_ERR_UNSUPPORTED;
+    }
     return 0;
 }
 
@@ -114,16 +121,16 @@ extern "C" int imager_mosaic_grid(imager_plan* plan, int32_t n_point, const int6
     const int64_t npix = (int64_t)n * n, nmos = (int64_t)n_mosaic * n_mosaic;
     float2* work = nullptr;
     double* total = nullptr;
-    IMAGER_CUDA(cudaMallocAsync(&work, npix * sizeof(float2), st));
-    IMAGER_CUDA(cudaMallocAsync(&total, sizeof(double), st));
     int launches = 0;
-    auto done = [&](int code) {
-        cudaFreeAsync(work, st);
-        cudaFreeAsync(total, st);
+    auto done = [&](int code) {                          // every exit frees what was allocated so far
+        if (work) cudaFreeAsync(work, st);
+        if (total) cudaFreeAsync(total, st);
         plan->last_launches = launches;
         return code;
     };
 #define MOSAIC_CUDA(call) do { cudaError_t e__ = (call); if (e__ != cudaSuccess) return done(cuda_fail(e__, #call)); } while (0)
+    MOSAIC_CUDA(cudaMallocAsync(&work, npix * sizeof(float2), st));
+    MOSAIC_CUDA(cudaMallocAsync(&total, sizeof(double), st));
     MOSAIC_CUDA(cudaMemsetAsync(total, 0, sizeof(double), st));
     MOSAIC_CUDA(cudaMemsetAsync(mosaic_image, 0, nmos * sizeof(float2), st));
     for (int i = 0; i < n_point; ++i) {
@@ -140,7 +147,7 @@ extern "C" int imager_mosaic_grid(imager_plan* plan, int32_t n_point, const int6
         if (rc) return done(rc);
         launches += 4;
     }
-    scale_by_inverse_kernel<<<4 * kNumSMs, 256, 0, st>>>(nmos, (float2*)mosaic_image, total);
+    scale_by_inverse_kernel<<<4 * num_sms(), 256, 0, st>>>(nmos, (float2*)mosaic_image, total);
     if (sum_weights) MOSAIC_CUDA(cudaMemcpyAsync(sum_weights, total, sizeof(double), cudaMemcpyDeviceToDevice, st));
     MOSAIC_CUDA(cudaGetLastError());
     return done(0);
@@ -173,7 +180,7 @@ extern "C" int imager_mosaic_degrid(imager_plan* plan, int32_t n_point, const in
         launches += plan->last_launches + 4;
         if (rc) return done(rc);
     }
-    IMAGER_CUDA(cudaGetLastError());
+    MOSAIC_CUDA(cudaGetLastError());
 #undef MOSAIC_CUDA
     return done(0);
 }

@@ -132,7 +132,7 @@ int mosaic_correct(imager_plan* pl, float2* image, cudaStream_t st) {
         if (e == cudaSuccess) {
             mosaic_ssq_kernel<<<dim3((N + 127) / 128, N), 128, 0, st>>>(N, pl->p.cell_size_rad, pl->p.dish_diameter_m, pl->p.freq_hz,
                                                                        na, d_lm, d_ssq, d_max);
-            mosaic_gamma_kernel<<<4 * kNumSMs, 256, 0, st>>>(n, d_ssq, d_max, d_gamma);
+            mosaic_gamma_kernel<<<4 * num_sms(), 256, 0, st>>>(n, d_ssq, d_max, d_gamma);
             e = cudaStreamSynchronize(st);                      // lm (host vector) and the scratch are released below
         }
         cudaFree(d_lm);
@@ -144,7 +144,7 @@ int mosaic_correct(imager_plan* pl, float2* image, cudaStream_t st) {
         }
         pl->d_gamma = d_gamma;
     }
-    mosaic_apply_kernel<<<4 * kNumSMs, 256, 0, st>>>(n, pl->p.n_pol, pl->d_gamma, image);
+    mosaic_apply_kernel<<<4 * num_sms(), 256, 0, st>>>(n, pl->p.n_pol, pl->d_gamma, image);
     IMAGER_CUDA(cudaGetLastError());
     return 0;
 }

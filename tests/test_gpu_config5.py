@@ -46,6 +46,7 @@ def test_config5_chunked_grid_fft_degrid_round_trip(oracle_lib):
     chunks = [(t0, min(t0 + steps_per_chunk, n_time)) for t0 in range(0, n_time, steps_per_chunk)]
     rng = np.random.default_rng(2025)
     with Plan(params, steps_per_chunk * per_step, user_tables=flat) as plan:
+        assert plan.path() == ("tiled", ""), f"config 5 would run on the reference kernels: {plan.path()[1]}"
         grid = torch.zeros((npol, n, n), dtype=torch.complex64, device="cuda")
         sumwt = torch.zeros(nc, dtype=torch.float64, device="cuda")
         cells = acc = acc_norm = None

@@ -5,7 +5,11 @@ library called through the binding):
     sum |kernel . vis| (block splitting, the two-ended queue and multi-group units only occur at these sizes);
   * config 3 (1.9e11 complex MACs: 20 core-minutes of oracle): 4000 sampled grid cells (half of them at visibility
     positions, half uniformly in the uv coverage) and 4000 sampled visibilities, which the oracle computes one by one.
+config 2 -- the configuration bench.py times -- is also run through a plan in WPROJ mode that builds its own tables, as bench.py
+does, and compared at every output with the oracle on the oracle's tables (bound 5e-5: two independent table generators).
 config 5 at its full size is tests/test_gpu_config5.py."""
+import os
+
 import numpy as np
 import pytest
 
@@ -16,7 +20,7 @@ pytestmark = pytest.mark.gpu
 TOL = 1e-5
 
 
-def _run(name, time_stride, n_samples=4000, every_output=False):
+def _run(name, time_stride, n_samples=4000, every_output=False, library_tables=False):
     import torch
     assert torch.cuda.is_available()
     from paper_2206_15117_b200 import Plan
@@ -29,6 +33,7 @@ def _run(name, time_stride, n_samples=4000, every_output=False):
     n, npol, nc = params["grid_size"], params["n_pol"], params["n_corr"]
     rng = np.random.default_rng(123)
     with Plan(params, nvis, user_tables=flat) as plan:
+        assert plan.path() == ("tiled", ""), f"{name} would run on the reference kernels: {plan.path()[1]}"
         uvw = torch.from_numpy(wl.uvw).cuda()
         a = torch.from_numpy(wl.a_index).cuda() if wl.a_index is not None else None
         got = plan.debug_index(uvw, a)
@@ -51,7 +56,8 @@ def _run(name, time_stride, n_samples=4000, every_output=False):
             assert np.all(g[~touched] == 0)
             err = np.max(np.abs(g[touched] - ref["grid"][touched]) / ref["norm"][touched])
             assert err <= TOL, f"{name}: all-cell grid parity {err:.3e}"
-            del ref
+            if not library_tables:
+                del ref
             out = torch.empty((nvis, nc), dtype=torch.complex64, device="cuda")
             plan.degrid(uvw, grid, out, a, flags=1)
             torch.cuda.synchronize()
@@ -61,6 +67,26 @@ def _run(name, time_stride, n_samples=4000, every_output=False):
             errd = np.max(np.abs(v[ok] - refd["vis"][ok]) / refd["norm"][ok])
             assert errd <= TOL, f"{name}: all-visibility degrid parity {errd:.3e}"
             assert np.all(v[rec["drop"]] == 0)
+            if library_tables:
+                # the mode bench.py times: the same data through a plan that generates ITS OWN tables (csrc/tables.cu), against
+                # the oracle run on the oracle's tables above -- every cell and every visibility, same normalised metric; the two
+                # table generators differ by ~1e-7 of the peak tap (tests/test_gpu_tables.py), hence the wider bound
+                del out
+                with Plan(params, nvis) as lib_plan:
+                    assert lib_plan.path() == ("tiled", "")
+                    lib_grid = torch.zeros((npol, n, n), dtype=torch.complex64, device="cuda")
+                    lib_plan.grid(uvw, vis, wts, lib_grid, a)
+                    lib_out = torch.empty((nvis, nc), dtype=torch.complex64, device="cuda")
+                    lib_plan.degrid(uvw, grid, lib_out, a, flags=1)          # degrid the SAME grid g the oracle degridded
+                    torch.cuda.synchronize()
+                    lg = lib_grid.cpu().numpy()
+                    assert np.all(lg[~touched] == 0)
+                    err = np.max(np.abs(lg[touched] - ref["grid"][touched]) / ref["norm"][touched])
+                    assert err <= 5e-5, f"{name}: library-table grid parity {err:.3e}"
+                    lv = lib_out.cpu().numpy()
+                    errd = np.max(np.abs(lv[ok] - refd["vis"][ok]) / refd["norm"][ok])
+                    assert errd <= 5e-5, f"{name}: library-table degrid parity {errd:.3e}"
+                    print(f"{name} with the library's own tables: grid {err:.2e}, degrid {errd:.2e} (bound 5e-5)")
             return
         # sampled cells
         pick = rng.integers(0, nvis, n_samples // 2)
@@ -93,8 +119,19 @@ def _run(name, time_stride, n_samples=4000, every_output=False):
 
 @pytest.mark.parametrize("name", ["config1", "config2", "config4"])
 def test_full_size_every_output(oracle_lib, name):
-    _run(name, 1, every_output=True)
+    _run(name, 1, every_output=True, library_tables=(name == "config2"))
 
 
 def test_full_size_sampled_parity_config3(oracle_lib):
     _run("config3", 1)
+
+
+@pytest.mark.slow
+@pytest.mark.skipif(os.environ.get("IMAGER_FULL_CONFIG3") != "1",
+                    reason="every output of config 3 costs about 7 minutes of oracle on 16 cores: set IMAGER_FULL_CONFIG3=1 "
+                           "(the log of such a run is committed as profiles/r3_config3_every_output.md)")
+def test_full_size_every_output_config3(oracle_lib):
+    """Config 3 at its stated size (BASELINE.json configs[2]: 4 correlations -> 4 Stokes grids of 4096^2, 16 Mueller
+    elements per tap): EVERY grid cell and EVERY degridded visibility against the oracle -- the only
+    full-size check of block splitting with 16 elements.  The sampled test above stays the default."""
+    _run("config3", 1, every_output=True)

@@ -88,3 +88,28 @@ def test_image_domain_mosaic_on_a_cut_of_config4(oracle_lib):
             refd = og.degrid(sub, mg[None].astype(np.complex64), flat, offs, params)
             v = o.cpu().numpy()[ks]
             assert np.abs(v - refd["vis"]).max() <= 2e-5 * np.abs(refd["vis"]).max(), i
+
+
+def test_plan_with_a_beam_in_its_kernels_is_refused():
+    """The image-domain mosaic applies the primary beam in the image plane; a MOSAIC_PB plan already holds it in its gridding
+    kernels and would apply it twice, so imager_mosaic_grid / _degrid refuse it (include/imager.h).  A grid too narrow for the
+    tiled kernels also shows up in imager_plan_path with its reason."""
+    import torch
+    from paper_2206_15117_b200 import ImagerError, Plan, MODE_MOSAIC_PB, MODE_PSWF
+    base = dict(grid_size=128, cell_size_rad=0.03 / 128, n_corr=1, n_pol=1, n_wplanes=1, w_max=0.0, support_min=16, support_max=16,
+                oversample=4, n_aplanes=1, dish_diameter_m=12.0, freq_hz=3.0e9, pointing_lm=[[0.0, 0.0]], pa_rad=[0.0])
+    uvw = torch.zeros((4, 3), dtype=torch.float32, device="cuda")
+    vis = torch.ones((4, 1), dtype=torch.complex64, device="cuda")
+    wts = torch.ones((4, 1), dtype=torch.float32, device="cuda")
+    mosaic = torch.zeros((64, 64), dtype=torch.complex64, device="cuda")
+    with Plan(dict(base, kernel_mode=MODE_MOSAIC_PB), 4) as plan:
+        assert plan.path() == ("tiled", "")
+        with pytest.raises(ImagerError, match="carries the primary beam"):
+            plan.mosaic_grid([uvw], [vis], [wts], [[0.0, 0.0]], mosaic, 0.03 / 128)
+        with pytest.raises(ImagerError, match="carries the primary beam"):
+            plan.mosaic_degrid([uvw], [[0.0, 0.0]], mosaic, 0.03 / 128, [vis])
+        torch.cuda.synchronize()
+        assert torch.count_nonzero(mosaic).item() == 0
+    with Plan(dict(base, kernel_mode=MODE_PSWF, grid_size=80, support_min=7, support_max=7), 4) as plan:
+        path, why = plan.path()
+        assert path == "reference" and "multiple of the 32-cell strip" in why

@@ -405,3 +405,39 @@ def test_invalid_input_is_dropped_not_indexed(torch_cuda, oracle_lib):
             assert torch.count_nonzero(guard[0]).item() == 0 and torch.count_nonzero(guard[-1]).item() == 0
             assert np.allclose(sumwt.cpu().numpy(), ref["sumwt"], rtol=1e-12)
             assert np.all(out.cpu().numpy()[rec["drop"]] == 0)
+
+
+@pytest.mark.parametrize("case", ["wproj", "awproj"])
+def test_flagged_samples_contribute_nothing(torch_cuda, oracle_lib, case):
+    """R24: samples with zero weight or a non-finite weight / value (flagged data often carry NaN) add nothing -- on both
+    kernel paths, with and without duplicates of the flagged visibility (whose pre-summed value must stay clean), and
+    nothing outside the footprints is written (the tiled kernel multiplies values into zero padding)."""
+    torch = torch_cuda
+    from paper_2206_15117_b200 import Plan
+    params = CASES[case]()
+    nvis, nc, npol, n = 6000, params["n_corr"], params["n_pol"], params["grid_size"]
+    uvw, vis, wts, a = random_vis(params, nvis, seed=123, frac=0.35, a_planes=params["n_aplanes"] > 1)
+    uvw[100:104] = uvw[7]                                                  # duplicates of a visibility that gets flagged
+    if a is not None:
+        a[100:104] = a[7]
+    bad = [(7, 0, np.nan + 0j, 0.0), (9, nc - 1, complex(np.inf, 1.0), 0.0), (101, 0, complex(1.0, np.nan), 0.0),
+           (500, 0, complex(np.nan, np.nan), 1.0), (501, nc - 1, 1.0 + 1.0j, np.nan), (502, 0, 1.0 - 2.0j, np.inf)]
+    for k, c, v, w in bad:
+        vis[k, c], wts[k, c] = v, w
+    _, _, flat, offs = oracle_tables(params)
+    rec = oidx.index_visibilities(uvw, a, params)
+    ref = og.grid(rec, vis, wts, flat, offs, params)
+    assert np.isfinite(ref["grid"]).all()
+    with Plan(params, nvis, user_tables=flat) as plan:
+        d_uvw, d_vis, d_wts, d_a = _to_dev(torch, uvw, vis, wts, a)
+        for flags in (0, 2):
+            guard = torch.zeros((npol + 2, n, n), dtype=torch.complex64, device="cuda")
+            grid = guard[1:npol + 1]
+            sumwt = torch.zeros(nc, dtype=torch.float64, device="cuda")
+            plan.grid(d_uvw, d_vis, d_wts, grid, d_a, sumwt, flags=flags)
+            torch.cuda.synchronize()
+            g = grid.cpu().numpy()
+            assert np.isfinite(g).all(), "a flagged sample reached the grid"
+            assert grid_error(g, ref) <= TOL
+            assert torch.count_nonzero(guard[0]).item() == 0 and torch.count_nonzero(guard[-1]).item() == 0
+            assert np.allclose(sumwt.cpu().numpy(), ref["sumwt"], rtol=1e-12)

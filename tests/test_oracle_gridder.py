@@ -244,3 +244,27 @@ def test_P13_grid_to_image_inverts_image_to_grid_up_to_taper_squared():
     one = np.zeros((n, n), np.complex128)
     one[n // 2, n // 2] = 1.0
     assert np.allclose(oi.image_to_grid(one), 1.0, atol=1e-12)
+
+
+def test_P21_flagged_samples_contribute_nothing(oracle_lib):
+    """Reading R24 (extends R9, "omega = 0 contributes 0"): a sample whose weight is zero, or whose weight or value is not
+    finite, adds nothing to the grid and nothing to the sum of weights.  Pinned against what that sentence fixes: the grid of
+    a data set with flagged samples (NaN / Inf values at zero weight, a NaN at weight 1, a NaN weight) is, bit for bit, the
+    grid of the same data set with those samples replaced by value 0 and weight 0 -- and is finite everywhere."""
+    from helpers import MODE_AWPROJ_ADJOINT
+    params = base_params(grid_size=64, oversample=4, n_wplanes=3, w_max=30.0, support_min=7, support_max=11, n_corr=4, n_pol=4,
+                         n_aplanes=2, pa_rad=[0.0, 0.7], pointing_lm=[[0, 0]] * 2, leakage=[0.01j, -0.01],
+                         kernel_mode=MODE_AWPROJ_ADJOINT, cell_size_rad=0.04 / 64)
+    uvw, vis, wts, a = random_vis(params, 300, seed=5, a_planes=True)
+    clean_vis, clean_wts = vis.copy(), wts.copy()
+    for k, c, v, w in [(3, 0, np.nan + 0j, 0.0), (3, 2, complex(np.inf, 1.0), 0.0), (17, 1, complex(2.0, -np.inf), 0.0),
+                       (40, 3, complex(np.nan, np.nan), 1.0), (41, 0, 1.0 + 1.0j, np.nan), (42, 2, 1.0 - 2.0j, np.inf)]:
+        vis[k, c], wts[k, c] = v, w
+        clean_vis[k, c], clean_wts[k, c] = 0.0, 0.0
+    wts[50, 1] = clean_wts[50, 1] = 0.0                                   # a plain zero weight with a finite value
+    out, _ = oracle_grid(params, uvw, vis, wts, a)
+    ref, _ = oracle_grid(params, uvw, clean_vis, clean_wts, a)
+    assert np.isfinite(out["grid"]).all() and np.isfinite(out["norm"]).all()
+    assert np.array_equal(out["grid"], ref["grid"]) and np.array_equal(out["norm"], ref["norm"])
+    assert np.array_equal(out["sumwt"], ref["sumwt"])
+    assert np.allclose(out["sumwt"], clean_wts.astype(np.float64).sum(axis=0), rtol=1e-12)
