@@ -24,16 +24,19 @@ __global__ void __launch_bounds__(kProbeThreads) lds64_probe_kernel(int iters, i
     float2 acc[kProbeUnroll];
 #pragma unroll
     for (int u = 0; u < kProbeUnroll; ++u) acc[u] = make_float2(0.f, 0.f);
-    const uint32_t base = (uint32_t)__cvta_generic_to_shared(buf) + (uint32_t)((warp * 32 + lane) * 8);
+    const uint32_t buf0 = (uint32_t)__cvta_generic_to_shared(buf);
+    const uint32_t off = (uint32_t)((warp * 32 + lane) * 8);             // a conflict-free 256-byte row per warp
     __syncthreads();
     const long long t0 = clock64();
     if (active) {
         for (int it = 0; it < iters; ++it) {
-            const uint32_t a = base;                                    // the same conflict-free 256-byte row every trip
+            // the address moves with the trip (8 rows of 2 KB apart) so that the compiler cannot merge the loads of
+            // successive trips; largest offset 8184 + 7 * 256 + 7 * 2048 < 32 KB
+            const uint32_t a = buf0 + off + (uint32_t)((it & 7) << 11);
 #pragma unroll
             for (int u = 0; u < kProbeUnroll; ++u) {
                 float x, y;
-                asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(x), "=f"(y) : "r"(a ^ (uint32_t)(u * 256)));
+                asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(x), "=f"(y) : "r"(a + (uint32_t)(u * 256)) : "memory");
                 acc[u].x += x;
                 acc[u].y += y;
             }
